@@ -1,0 +1,76 @@
+/* bz_oracle.h -- CPU oracle for the per-zone nuclear burn.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may call this.  It shares no code with the CUDA path (paper_1711_06203_b200/).
+ *
+ * What it computes (section 4: "do the entire ODE integration ... all
+ * righthand side and Jacobian evaluations and the timestepping itself"; ref [33] VODE,
+ * PAPER.md L184): for every zone independently, integrate
+ *     dY_i/dt = sum_k D_ik R_k ,   dT/dt = (N_A MeV / c_v) sum_k Q_k R_k
+ * over one hydro step dt with a variable-coefficient, variable-order (1..5) BDF in
+ * Nordsieck form, Newton iteration on I - gamma*J with an analytic dense Jacobian and a
+ * LINPACK-style dense LU (dgefa/dgesl).  The paper prints none of the formulas; the
+ * algorithm ("BZ-BDF v1") is the reading recorded in DESIGN.md section 3, taken from
+ * SURVEY.md section 8(c) C.1-C.2, and is followed here step by step in that notation.
+ *
+ * Parity status of the parts (pins live in tests/test_oracle_*.py, all -m "not gpu"):
+ *   rate law, RHS, Jacobian, LU/solve, exp/log, BDF coefficients, order of accuracy,
+ *   the integrator (closed forms, invariants, brute-force implicit Euler, scipy Radau):
+ *   pinned.   The VALUES of the step/order heuristics constants (BIAS1..3, THRESH,
+ *   ETAMAX, ...): parity unpinned -- any values pass the pins; they are fixed by
+ *   DESIGN.md section 3 only.
+ */
+#ifndef BZ_ORACLE_H
+#define BZ_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORC_NMAX 32   /* max unknowns n = nspec + 1 */
+#define ORC_KMAX 256  /* max reactions */
+
+typedef struct {
+  int32_t nspec, nreac;
+  const double *aion;        /* [N]    mass numbers A_i                                  */
+  const int32_t *reactant;   /* [K][3] reactant particle species ids, -1 unused          */
+  const int32_t *stoich_id;  /* [K][4] species whose Y changes, -1 unused                */
+  const double *stoich_dy;   /* [K][4] change per reaction event                         */
+  const double *rate_A, *rate_n, *rate_B; /* [K] lambda = A T9^n exp(-B T9^(-1/3))       */
+  const double *q_mev;       /* [K]    MeV per event                                     */
+  double cv;                 /* erg/g/K                                                  */
+} orc_net_desc;
+
+typedef struct {
+  int32_t norm_lanes;  /* 1,2,4,8,16,32: association of the WRMS-norm sum */
+  int32_t fixed_q;     /* test hook: 0 = adaptive; q>0 = fixed order, fixed step, no error test */
+  double fixed_h;      /* test hook: the fixed step                                       */
+  const double *z_init;/* test hook: [(fixed_q+1)][n] initial Nordsieck array (scaled by fixed_h) */
+  int32_t nthreads;    /* OpenMP threads over zones; <=0 = runtime default                */
+} orc_opts;
+
+/* counters[8] = {nst, nrhs, njac, nlu, nsolve, netf, ncfn, nfailzones} summed over zones */
+int orc_burn(const orc_net_desc *d, int64_t nz, const double *rho, const double *T,
+             const double *X /*[N][nz]*/, double dt, double rtol, double atol,
+             double *T_out, double *X_out, int32_t *nsteps, const orc_opts *opts,
+             uint64_t counters[8]);
+
+/* pieces exposed for the pins */
+int orc_rates(const orc_net_desc *d, double rho, const double *y /*[n]*/, double *f /*[n]*/,
+              double *J /*[n*n] row-major or NULL*/);
+double orc_exp(double x);
+double orc_log(double x);
+/* a: [n*n] row-major, overwritten by LU (multipliers +l_ik below, U above, on the diagonal
+ * the pivots); inv[n] = 1/pivot; ipvt[n].  returns 0, or k+1 if pivot k is exactly zero. */
+int orc_lu_factor(int n, double *a, int32_t *ipvt, double *inv);
+void orc_lu_solve(int n, const double *a, const int32_t *ipvt, const double *inv, double *b);
+/* l[0..q], for step h and history tau[1..5] (tau[0] unused) */
+void orc_bdf_coeffs(int q, double h, const double *tau, double *l);
+double orc_wrms(int n, const double *v, const double *w, int lanes);
+int orc_max_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
