@@ -1,0 +1,119 @@
+/* burnzones.h -- C ABI of libburn: the per-zone nuclear burn on one B200 (sm_100a).
+ *
+ * The operation (section 4): "do the entire ODE integration on the GPU, i.e.,
+ * the data for a patch of zones is passed to the GPU, all righthand side and Jacobian
+ * evaluations and the timestepping itself is done on the GPU, and once the burning in all
+ * zones is completed, we access the data as needed"; the integrator is VODE (ref. [33],
+ * PAPER.md L184); "rates and integration strategy are decoupled" (L83).  The call list is
+ * BASELINE.json:north_star's: net_create(rates, Q-values, isotope masses),
+ * burn_zones(rho[], T[], X[][], dt, rtol, atol, out T[], out X[], out nsteps[], stream),
+ * net_destroy.  The exact model and algorithm ("BZ-BDF v1") are DESIGN.md section 3.
+ *
+ * Conventions
+ *   - plain C, no exceptions, no abort; every call returns 0 or a negative bz_status.
+ *   - "HOST" / "DEVICE" says where a pointer must point.  DEVICE arrays and the stream are
+ *     owned by the caller (PyTorch allocates them); the library owns the bz_net handle, its
+ *     device-side tables and its scratch (work-queue counter, counters, staging buffers).
+ *   - layout: structure of arrays, species-major, zone index fastest:  X[i*nz + z].
+ *     Zone order is the grid's x-fastest order but the library attaches no meaning to it.
+ *   - burn_zones only enqueues work on `cuda_stream` and returns; it never synchronises the
+ *     device.  Outputs are valid after the caller synchronises the stream.
+ *   - exact aliasing T_out == T and X_out == X is allowed (each zone is read completely before
+ *     it is written); partial overlap is undefined.
+ *   - there is no CPU fallback: without a CUDA device every compute call returns BZ_ERR_CUDA.
+ */
+#ifndef BURNZONES_H
+#define BURNZONES_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bz_net bz_net; /* opaque, owned by the library */
+
+typedef enum {
+  BZ_OK = 0,
+  BZ_ERR_NULL = -1,    /* a required pointer is NULL                                          */
+  BZ_ERR_SIZE = -2,    /* nspec not in 1..31, nreac not in 1..256, nz < 0                     */
+  BZ_ERR_NETWORK = -3, /* species id out of range, A_i <= 0, cv <= 0, rate_A <= 0, non-finite
+                          coefficient, reaction without reactant, repeated stoichiometry id    */
+  BZ_ERR_SCALAR = -4,  /* dt <= 0, rtol <= 0, atol < 0, or non-finite                         */
+  BZ_ERR_CUDA = -5,    /* CUDA runtime error; the cudaError_t is in bz_last_cuda_error()      */
+  BZ_ERR_NOMEM = -6    /* host or device allocation failed                                    */
+} bz_status;
+
+/* Network descriptor.  All pointers are HOST pointers and are
+ * copied; the caller may free them when net_create returns.
+ *   rate law   lambda_k = rate_A * T9^rate_n * exp(-rate_B / T9^(1/3)),  T9 = T / 1e9
+ *              R_k = lambda_k * rho^(m_k - 1) * prod_{p in reactant[k]} Y_p / prod_i nu_ik!
+ *   ODEs       dY_i/dt = sum_k stoich_dy[k][.] R_k ;  dT/dt = (N_A MeV / cv) sum_k q_mev[k] R_k
+ */
+typedef struct {
+  int32_t nspec, nreac;      /* N (1..31), K (1..256)                                          */
+  const double *aion;        /* [N]    mass numbers A_i ("isotope masses"); Y_i = X_i / A_i    */
+  const int32_t *reactant;   /* [K][3] species id of each reactant particle, -1 = unused;
+                                        identical particles repeated (3-alpha = {0,0,0})       */
+  const int32_t *stoich_id;  /* [K][4] species whose Y changes, -1 = unused, ids distinct      */
+  const double *stoich_dy;   /* [K][4] net change of Y per reaction event                      */
+  const double *rate_A, *rate_n, *rate_B; /* [K]                                              */
+  const double *q_mev;       /* [K]    Q-values, MeV per reaction event                        */
+  double cv;                 /* specific heat, erg g^-1 K^-1, constant                         */
+} bz_net_desc;
+
+/* Validate, flatten and upload a network.  *out receives the handle. */
+int net_create(const bz_net_desc *desc, bz_net **out);
+
+/* Integrate every zone's network over [0, dt] (steps a1-a9 of DESIGN.md section 2).
+ *   nz             number of zones (0 is a no-op)
+ *   rho, T         DEVICE [nz]       density g/cc, temperature K (inputs)
+ *   X              DEVICE [N][nz]    mass fractions of the N evolved species (input)
+ *   dt, rtol, atol burn interval (s); relative tolerance; absolute tolerance on Y (mol/g)
+ *   T_out, X_out   DEVICE [nz], [N][nz]   results
+ *   nsteps         DEVICE [nz] int32: accepted BDF steps, or a per-zone failure code
+ *                    -1  more than 10 Newton failures on one step
+ *                    -2  7 error-test failures on one step
+ *                    -3  100000 steps taken without reaching dt
+ *                    -4  invalid input zone (non-finite, rho <= 0 or T <= 0): outputs = inputs
+ *                  failed zones hold the last accepted state; they do not fail the call.
+ *   cuda_stream    cudaStream_t (as void*) on which all work is enqueued
+ */
+int burn_zones(const bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
+               double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
+               void *cuda_stream);
+
+/* The same burn with HOST arrays (pinned memory recommended): copies inputs to library-owned
+ * device staging, runs burn_zones, copies the three outputs back, all on `cuda_stream`, and
+ * returns without synchronising.  This is the end-to-end path bench.py times. */
+int burn_zones_host(bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
+                    double dt, double rtol, double atol, double *T_out, double *X_out,
+                    int32_t *nsteps, void *cuda_stream);
+
+int net_destroy(bz_net *net);
+
+/* Totals over the zones of the most recent burn_zones on this handle:
+ * out[8] = {nst, nrhs, njac, nlu, nsolve, netf, ncfn, nfailzones} (HOST).  Synchronises
+ * `cuda_stream` (it has to read the device counters). */
+int bz_get_counters(const bz_net *net, void *cuda_stream, uint64_t out[8]);
+
+/* Association of the WRMS-norm sum used by the kernel selected for this network
+ * (DESIGN.md 3.6): 1, 4, 8, 16 or 32 interleaved partial sums combined by an xor butterfly.
+ * Returns the lane count (>0) or a negative bz_status. */
+int bz_norm_lanes(const bz_net *net);
+
+/* Name of the kernel variant burn_zones launches for this network (static string). */
+const char *bz_kernel_name(const bz_net *net);
+
+/* Last cudaError_t seen by this thread inside the library (0 = cudaSuccess). */
+int bz_last_cuda_error(void);
+
+/* FP64 peak probe: runs a DFMA-chain kernel on every SM for `iters` iterations of 8x32
+ * independent fused multiply-adds per thread and returns the measured TFLOP/s (FMA = 2) in
+ * *tflops and the elapsed milliseconds in *ms.  Synchronises the stream.  Used by bench.py to
+ * report the denominator of the roofline. */
+int bz_fp64_peak_probe(int64_t iters, void *cuda_stream, double *tflops, double *ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BURNZONES_H */

@@ -1,0 +1,197 @@
+"""ctypes binding of libburn.so -- argument marshalling only; every step of the burn runs in the
+CUDA kernels behind the C ABI (include/burnzones.h)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
+EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_host", "net_destroy", "bz_get_counters",
+                    "bz_norm_lanes", "bz_kernel_name", "bz_last_cuda_error", "bz_fp64_peak_probe")
+_STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
+           -5: "CUDA runtime error", -6: "out of memory"}
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+class BurnError(RuntimeError):
+    def __init__(self, code, what, cuda_error=0):
+        self.code = code
+        self.cuda_error = cuda_error
+        extra = f" (cudaError_t {cuda_error})" if code == -5 else ""
+        super().__init__(f"{what} failed: {_STATUS.get(code, 'unknown')} [{code}]{extra}")
+
+
+class _Desc(C.Structure):
+    _fields_ = [("nspec", C.c_int32), ("nreac", C.c_int32), ("aion", _dp), ("reactant", _ip),
+                ("stoich_id", _ip), ("stoich_dy", _dp), ("rate_A", _dp), ("rate_n", _dp),
+                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double)]
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "libburn.so")
+
+
+_lib = None
+
+
+def _L():
+    """Load libburn.so.  It must have been built (python -m paper_1711_06203_b200.build or
+    __graft_entry__.build()); a missing library is an error, never a fallback."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: build it with __graft_entry__.build(); "
+                              "there is no CPU fallback for the burn")
+        lib = C.CDLL(path)
+        vp = C.c_void_p
+        lib.net_create.restype = C.c_int
+        lib.net_create.argtypes = [C.POINTER(_Desc), C.POINTER(vp)]
+        lib.net_destroy.restype = C.c_int
+        lib.net_destroy.argtypes = [vp]
+        sig = [vp, C.c_int64, vp, vp, vp, C.c_double, C.c_double, C.c_double, vp, vp, vp, vp]
+        lib.burn_zones.restype = C.c_int
+        lib.burn_zones.argtypes = sig
+        lib.burn_zones_host.restype = C.c_int
+        lib.burn_zones_host.argtypes = sig
+        lib.bz_get_counters.restype = C.c_int
+        lib.bz_get_counters.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
+        lib.bz_norm_lanes.restype = C.c_int
+        lib.bz_norm_lanes.argtypes = [vp]
+        lib.bz_kernel_name.restype = C.c_char_p
+        lib.bz_kernel_name.argtypes = [vp]
+        lib.bz_last_cuda_error.restype = C.c_int
+        lib.bz_fp64_peak_probe.restype = C.c_int
+        lib.bz_fp64_peak_probe.argtypes = [C.c_int64, vp, _dp, _dp]
+        _lib = lib
+    return _lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise BurnError(rc, what, _L().bz_last_cuda_error())
+
+
+class Net:
+    """Handle returned by net_create (owns the library-side bz_net)."""
+
+    def __init__(self, handle, nspec, nreac):
+        self._h = handle
+        self.nspec = nspec
+        self.nreac = nreac
+
+    @property
+    def norm_lanes(self) -> int:
+        return int(_L().bz_norm_lanes(self._h))
+
+    @property
+    def kernel_name(self) -> str:
+        return _L().bz_kernel_name(self._h).decode()
+
+    def close(self):
+        if self._h is not None:
+            _L().net_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def net_create(net=None, *, aion=None, reactant=None, stoich_id=None, stoich_dy=None, rate_A=None,
+               rate_n=None, rate_B=None, q_mev=None, cv=None) -> Net:
+    """net_create(rates, Q-values, isotope masses): `net` is any object with those fields
+    (e.g. workloads.Network), or pass them as keywords."""
+    g = (lambda k, v: v if v is not None else getattr(net, k))
+    keep = dict(aion=_f64(g("aion", aion)), reactant=_i32(g("reactant", reactant)),
+                stoich_id=_i32(g("stoich_id", stoich_id)), stoich_dy=_f64(g("stoich_dy", stoich_dy)),
+                rate_A=_f64(g("rate_A", rate_A)), rate_n=_f64(g("rate_n", rate_n)),
+                rate_B=_f64(g("rate_B", rate_B)), q_mev=_f64(g("q_mev", q_mev)))
+    N, K = keep["aion"].shape[0], keep["rate_A"].shape[0]
+    if keep["reactant"].shape != (K, 3) or keep["stoich_id"].shape != (K, 4) or keep["stoich_dy"].shape != (K, 4):
+        raise ValueError("reactant must be [K,3], stoich_id/stoich_dy [K,4]")
+    for k in ("rate_n", "rate_B", "q_mev"):
+        if keep[k].shape != (K,):
+            raise ValueError(f"{k} must be [K]")
+    d = _Desc(N, K, keep["aion"].ctypes.data_as(_dp), keep["reactant"].ctypes.data_as(_ip),
+              keep["stoich_id"].ctypes.data_as(_ip), keep["stoich_dy"].ctypes.data_as(_dp),
+              keep["rate_A"].ctypes.data_as(_dp), keep["rate_n"].ctypes.data_as(_dp),
+              keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp),
+              float(g("cv", cv)))
+    h = C.c_void_p()
+    _check(_L().net_create(C.byref(d), C.byref(h)), "net_create")
+    return Net(h, N, K)
+
+
+def net_destroy(net: Net) -> None:
+    net.close()
+
+
+def _stream_ptr(stream):
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def burn_zones(net: Net, rho, T, X, dt, rtol, atol, T_out=None, X_out=None, nsteps=None, stream=None):
+    """Device tensors in, device tensors out (torch, float64, contiguous; X is [nspec, nz]).
+    Enqueues on `stream` (default: torch's current stream) and returns without synchronising."""
+    import torch
+    nz = rho.shape[0]
+    for name, t, shape in (("rho", rho, (nz,)), ("T", T, (nz,)), ("X", X, (net.nspec, nz))):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
+            raise ValueError(f"{name} must be a contiguous float64 CUDA tensor of shape {shape}")
+    if T_out is None:
+        T_out = torch.empty_like(T)
+    if X_out is None:
+        X_out = torch.empty_like(X)
+    if nsteps is None:
+        nsteps = torch.empty(nz, dtype=torch.int32, device=rho.device)
+    for name, t, dt_, shape in (("T_out", T_out, torch.float64, (nz,)), ("X_out", X_out, torch.float64, (net.nspec, nz)),
+                                ("nsteps", nsteps, torch.int32, (nz,))):
+        if not (t.is_cuda and t.dtype == dt_ and t.is_contiguous() and tuple(t.shape) == shape):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {shape}")
+    p = lambda t: C.c_void_p(t.data_ptr())
+    _check(_L().burn_zones(net._h, nz, p(rho), p(T), p(X), float(dt), float(rtol), float(atol),
+                           p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones")
+    return T_out, X_out, nsteps
+
+
+def burn_zones_host(net: Net, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, stream=None):
+    """Host (ideally pinned) torch tensors or numpy arrays in and out; H2D + burn + D2H are
+    enqueued on `stream`.  The caller synchronises."""
+    nz = rho.shape[0]
+
+    def ptr(a):
+        return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+    _check(_L().burn_zones_host(net._h, nz, ptr(rho), ptr(T), ptr(X), float(dt), float(rtol), float(atol),
+                                ptr(T_out), ptr(X_out), ptr(nsteps), _stream_ptr(stream)), "burn_zones_host")
+    return T_out, X_out, nsteps
+
+
+def get_counters(net: Net, stream=None) -> dict:
+    out = (C.c_uint64 * 8)()
+    _check(_L().bz_get_counters(net._h, _stream_ptr(stream), out), "bz_get_counters")
+    return dict(zip(COUNTER_NAMES, (int(v) for v in out)))
+
+
+def fp64_peak_probe(iters: int = 4000, stream=None):
+    """Measured DFMA throughput of this GPU: returns (TFLOP/s, milliseconds)."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(_L().bz_fp64_peak_probe(int(iters), _stream_ptr(stream), C.byref(tf), C.byref(ms)), "bz_fp64_peak_probe")
+    return tf.value, ms.value

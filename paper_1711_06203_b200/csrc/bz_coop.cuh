@@ -1,0 +1,85 @@
+// bz_coop.cuh -- cooperative burn kernel: LANES threads of a warp integrate one zone.
+//
+// Mapping: lane i of a group owns component i of every n-vector
+// (Nordsieck rows, weights, corrections) and ROW i of the Newton matrix P = I - gamma*J, all in
+// registers.  A warp holds 32/LANES zones.  Groups pull zones from a global atomic work queue
+// (step a2: compaction against step-count divergence -- a group that finishes its zone fetches
+// the next one, so co-resident zones never wait for the slowest of a fixed batch).
+//   a3/a4 rates + Jacobian: reactions are dealt round-robin to lanes (one exp each), the
+//         per-reaction rate and partials go through shared memory, then lane i gathers row i.
+//   a5    LU: implicit row pivoting (rows never move; each lane carries its LINPACK position
+//         `pos`), pivot search by a 64-bit max butterfly, pivot row broadcast through shared
+//         memory, rank-1 update of the lane's own row with fma.
+//   a6    solves: dgesl order; the pivot component is broadcast by shuffle.
+//   a7/a8 BDF bookkeeping: per lane on its own component; step/order control is computed
+//         redundantly by every lane of the group (identical bits, no communication).
+// The floating-point operation sequence per component is the one fixed in DESIGN.md 3.6, so the
+// results are bit-identical to the CPU oracle run with norm_lanes = LANES.
+#pragma once
+#include <cstdint>
+#include "bz_math.cuh"
+
+namespace bz {
+
+// ---- constants of BZ-BDF v1 ---------------------------------------------------
+constexpr int QMAX = 5, MAXCOR = 3, MXNCF = 10, MXNEF = 7, MXSTEP = 100000;
+constexpr double NTOL = 0.1, CRDOWN = 0.3, RDIV = 2.0, ETACF = 0.25;
+constexpr double BIAS1 = 4.0, BIAS2 = 6.0, BIAS3 = 10.0, ADDON = 1e-6, THRESH = 1.5;
+constexpr double ETAMIN = 0.1, ETAMXF = 0.2, ETAMX1 = 1e4, ETAMAX = 2.0, SLIVER = 1e-6;
+
+// flat network tables in device memory (built by net_create)
+struct DevNet {
+  int N, n, K, nterm, ncl;
+  double fac;             // N_A MeV / cv
+  const double *dbl;      // lnA[K] en[K] B[K] Q[K] invsym[K] aion[N] sp_dy[nterm]
+  const int *itab;        // rp[4K] sp_off[N+1] sp_k[nterm] cl_off[N+1] cl_ks[ncl]
+  int ndbl, nint;
+};
+
+struct BurnArgs {
+  long long nz;
+  const double *rho, *T, *X;
+  double dt, rtol, atol;
+  double *T_out, *X_out;
+  int *nsteps;
+  unsigned long long *queue;     // work-queue head
+  unsigned long long *counters;  // [8]
+};
+
+__device__ __forceinline__ double inv_small_int(int p) {  // 1.0/p, p = 1..7, correctly rounded
+  switch (p) {
+    case 1: return 1.0;
+    case 2: return 1.0 / 2.0;
+    case 3: return 1.0 / 3.0;
+    case 4: return 1.0 / 4.0;
+    case 5: return 1.0 / 5.0;
+    case 6: return 1.0 / 6.0;
+    default: return 1.0 / 7.0;
+  }
+}
+__device__ __forceinline__ double factorial_(int p) {  // p = 0..7
+  switch (p) {
+    case 0: case 1: return 1.0;
+    case 2: return 2.0;
+    case 3: return 6.0;
+    case 4: return 24.0;
+    case 5: return 120.0;
+    case 6: return 720.0;
+    default: return 5040.0;
+  }
+}
+// eta = 1 / ((bias*E)^(1/p) + ADDON), root through the own exp/log
+__device__ __forceinline__ double eta_of(double E, double bias, int p) {
+  const double v = bias * E;
+  const double root = (v > 1e-300) ? exp_(log_(v) * inv_small_int(p)) : 0.0;
+  return 1.0 / (root + ADDON);
+}
+
+template <int NEQ, int LANES>
+struct CoopSmem {
+  // per-group scratch, in doubles
+  static constexpr int LD = LANES + 1;
+  __host__ __device__ static constexpr int per_group(int K) { return LANES /*ysh*/ + 5 * K /*R,dRdT,dRdY*/ + LANES * LD /*M*/ + 2 * LANES /*urow*/ + LANES /*xs*/; }
+};
+
+}  // namespace bz

@@ -1,0 +1,183 @@
+// bz_coop_kernel.cuh -- body of the cooperative burn kernel (see bz_coop.cuh for the mapping).
+#pragma once
+#include "bz_coop.cuh"
+
+namespace bz {
+
+template <int NEQ, int LANES>
+struct Group {
+  static constexpr int LD = LANES + 1;
+  // identity of this lane
+  unsigned gmask;  // lanes of my group within the warp
+  int lig;         // lane in group = component index
+  // tables in shared memory (per block)
+  int N, n, K;
+  double fac, inv_n;
+  const double *lnA, *en, *B, *Q, *invsym, *aion, *sp_dy;
+  const int *rp, *sp_off, *sp_k, *cl_off, *cl_ks;
+  // per-group scratch in shared memory
+  double *ysh, *R, *dRdT, *dRdY, *M, *urow, *xs;
+
+  __device__ __forceinline__ void sync() const { __syncwarp(gmask); }
+
+  __device__ __forceinline__ double gsum(double v) const {
+#pragma unroll
+    for (int s = LANES / 2; s >= 1; s >>= 1) v = v + __shfl_xor_sync(gmask, v, s, LANES);
+    return v;
+  }
+  __device__ __forceinline__ unsigned long long gmax(unsigned long long v) const {
+#pragma unroll
+    for (int s = LANES / 2; s >= 1; s >>= 1) {
+      unsigned long long o = __shfl_xor_sync(gmask, v, s, LANES);
+      v = o > v ? o : v;
+    }
+    return v;
+  }
+  __device__ __forceinline__ int gmin(int v) const {
+#pragma unroll
+    for (int s = LANES / 2; s >= 1; s >>= 1) {
+      int o = __shfl_xor_sync(gmask, v, s, LANES);
+      v = o < v ? o : v;
+    }
+    return v;
+  }
+  // group-relative ballot
+  __device__ __forceinline__ unsigned gballot(bool p) const {
+    unsigned b = __ballot_sync(gmask, p);
+    if (LANES == 32) return b;
+    return (b >> ((threadIdx.x & 31) & ~(LANES - 1))) & ((1u << (LANES & 31)) - 1u);
+  }
+  __device__ __forceinline__ bool gany(bool p) const { return gballot(p) != 0u; }
+  __device__ __forceinline__ double bcast(double v, int src) const { return __shfl_sync(gmask, v, src, LANES); }
+
+  // WRMS norm, association = LANES interleaved partial sums + xor butterfly
+  __device__ __forceinline__ double wrms(double v, double w) const {
+    const double d = v * w;
+    const double s = gsum(d * d);
+    return sqrt(s * inv_n);
+  }
+
+  // a3 (+a4): f (own component) and, if WITH_J, row `lig` of J left in M (shared memory).
+  template <bool WITH_J>
+  __device__ __forceinline__ double rates(double rho, double y) {
+    sync();  // previous readers of the scratch are done
+    if (lig < n) ysh[lig] = y;
+    sync();
+    const double T = ysh[N];
+    const double T9 = T * 1e-9;
+    const double lnT9 = log_(T9);
+    const double t13 = exp_(lnT9 * (-1.0 / 3.0));
+    const double t13third = t13 * (1.0 / 3.0);
+    const double invT = 1.0 / T;
+    const double rho2 = rho * rho;
+    for (int k = lig; k < K; k += LANES) {
+      const int4 rpk = reinterpret_cast<const int4 *>(rp)[k];
+      const int m = rpk.x & 0xff;
+      const int r0 = rpk.y & 0xff, r1 = (rpk.y >> 8) & 0xff, r2 = (rpk.y >> 16) & 0xff;
+      const double arg = fma_(-B[k], t13, fma_(en[k], lnT9, lnA[k]));
+      const double lam = exp_(arg);
+      const double pref = (lam * (m == 1 ? 1.0 : (m == 2 ? rho : rho2))) * invsym[k];
+      const double y0 = ysh[r0];
+      const double v0 = fabs(y0);
+      double Rk, d0, d1 = 0.0, d2 = 0.0;
+      bool neg0 = y0 < 0.0, neg1 = false, neg2 = false;
+      if (m == 1) {
+        Rk = pref * v0;
+        d0 = pref;
+      } else if (m == 2) {
+        const double y1 = ysh[r1];
+        const double v1 = fabs(y1);
+        neg1 = y1 < 0.0;
+        Rk = (pref * v0) * v1;
+        if (r1 == r0) {
+          d0 = pref * (v1 + v0);
+        } else {
+          d0 = pref * v1;
+          d1 = pref * v0;
+        }
+      } else {
+        const double y1 = ysh[r1], y2 = ysh[r2];
+        const double v1 = fabs(y1), v2 = fabs(y2);
+        neg1 = y1 < 0.0;
+        neg2 = y2 < 0.0;
+        Rk = ((pref * v0) * v1) * v2;
+        const double P0 = v1 * v2, P1 = v0 * v2, P2 = v0 * v1;
+        // slots = distinct species in order of first appearance
+        double s0 = P0;
+        if (r1 == r0) s0 = s0 + P1;
+        if (r2 == r0) s0 = s0 + P2;
+        d0 = pref * s0;
+        if (r1 != r0) {
+          double s1 = P1;
+          if (r2 == r1) s1 = s1 + P2;
+          d1 = pref * s1;
+          if (r2 != r0 && r2 != r1) d2 = pref * P2;
+        } else if (r2 != r0) {
+          d1 = pref * P2;
+        }
+      }
+      const bool anyneg = neg0 | neg1 | neg2;
+      if (anyneg) Rk = -Rk;  // reading s19: odd, monotone extension to Y < 0
+      R[k] = Rk;
+      if (WITH_J) {
+        // sign of the partial w.r.t. a slot's species: flipped unless that species is negative
+        const int c0 = rpk.z & 0xff, c1 = (rpk.z >> 8) & 0xff, c2 = (rpk.z >> 16) & 0xff;
+        const int nslot = (rpk.x >> 8) & 0xff;
+        if (anyneg) {
+          if (!(ysh[c0] < 0.0)) d0 = -d0;
+          if (nslot > 1 && !(ysh[c1] < 0.0)) d1 = -d1;
+          if (nslot > 2 && !(ysh[c2] < 0.0)) d2 = -d2;
+        }
+        dRdY[3 * k + 0] = d0;
+        dRdY[3 * k + 1] = d1;
+        dRdY[3 * k + 2] = d2;
+        const double g = fma_(B[k], t13third, en[k]);
+        dRdT[k] = (Rk * g) * invT;
+      }
+    }
+    sync();
+    double f = 0.0;
+    if (lig < N) {
+      const int e = sp_off[lig + 1];
+      for (int t = sp_off[lig]; t < e; t++) f = fma_(sp_dy[t], R[sp_k[t]], f);
+    } else if (lig == N) {
+      double s = 0.0;
+      for (int k = 0; k < K; k++) s = fma_(Q[k], R[k], s);
+      f = fac * s;
+    }
+    if (WITH_J) {
+      double *row = M + lig * LD;
+      if (lig < n)
+        for (int j = 0; j < n; j++) row[j] = 0.0;
+      double jt = 0.0;
+      if (lig < N) {
+        const int e = sp_off[lig + 1];
+        for (int t = sp_off[lig]; t < e; t++) {
+          const int k = sp_k[t];
+          const double dy = sp_dy[t];
+          const int4 rpk = reinterpret_cast<const int4 *>(rp)[k];
+          const int nslot = (rpk.x >> 8) & 0xff;
+          const int c0 = rpk.z & 0xff, c1 = (rpk.z >> 8) & 0xff, c2 = (rpk.z >> 16) & 0xff;
+          row[c0] = fma_(dy, dRdY[3 * k], row[c0]);
+          if (nslot > 1) row[c1] = fma_(dy, dRdY[3 * k + 1], row[c1]);
+          if (nslot > 2) row[c2] = fma_(dy, dRdY[3 * k + 2], row[c2]);
+          row[N] = fma_(dy, dRdT[k], row[N]);
+        }
+        // my column of the temperature row: sum_k Q_k dR_k/dY_lig, k ascending
+        const int ce = cl_off[lig + 1];
+        for (int c = cl_off[lig]; c < ce; c++) {
+          const int ks = cl_ks[c];
+          jt = fma_(Q[ks & 0xffff], dRdY[3 * (ks & 0xffff) + (ks >> 16)], jt);
+        }
+      } else if (lig == N) {
+        for (int k = 0; k < K; k++) jt = fma_(Q[k], dRdT[k], jt);
+      }
+      sync();  // rows of the species are complete before the T row is written
+      if (lig < n) M[N * LD + lig] = fac * jt;
+      sync();
+    }
+    return f;
+  }
+};
+
+}  // namespace bz

@@ -1,0 +1,76 @@
+// bz_math.cuh -- device-side exp/log with a fixed IEEE operation sequence (DESIGN.md 3.6,
+// item 3).  Compiled with -fmad=false: every fused operation is an explicit fma().
+// libdevice exp/log are NOT used on the burn path: their results differ from any host libm by
+// an ulp in a few per cent of calls, which the BDF controller amplifies.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace bz {
+
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+
+// exp(x) = 2^k exp(r), r = x - k ln2 (two-piece ln2), exp(r) = sum_{j<=13} r^j/j! by Horner.
+// x < -700 -> 0, x > 700 -> +inf, so the scaling by 2^k is exact (no subnormal results).
+__device__ __forceinline__ double exp_(double x) {
+  constexpr double LOG2E = 1.4426950408889634;
+  constexpr double LN2_HI = 0x1.62e42fee00000p-1;
+  constexpr double LN2_LO = 0x1.a39ef35793c76p-33;
+  if (!(x >= -700.0)) return (x != x) ? x : 0.0;
+  if (x > 700.0) return __longlong_as_double(0x7ff0000000000000LL);
+  const double kd = rint(x * LOG2E);
+  double r = fma_(-kd, LN2_HI, x);
+  r = fma_(-kd, LN2_LO, r);
+  double p = 1.0 / 6227020800.0;
+  p = fma_(p, r, 1.0 / 479001600.0);
+  p = fma_(p, r, 1.0 / 39916800.0);
+  p = fma_(p, r, 1.0 / 3628800.0);
+  p = fma_(p, r, 1.0 / 362880.0);
+  p = fma_(p, r, 1.0 / 40320.0);
+  p = fma_(p, r, 1.0 / 5040.0);
+  p = fma_(p, r, 1.0 / 720.0);
+  p = fma_(p, r, 1.0 / 120.0);
+  p = fma_(p, r, 1.0 / 24.0);
+  p = fma_(p, r, 1.0 / 6.0);
+  p = fma_(p, r, 1.0 / 2.0);
+  p = fma_(p, r, 1.0);
+  p = fma_(p, r, 1.0);
+  const int k = (int)kd;  // |k| <= 1010
+  const double scale = __longlong_as_double((long long)(k + 1023) << 52);
+  return p * scale;  // exact: p in [0.7, 1.42], result normal
+}
+
+// log(x), x > 0 normal: x = m 2^e with m in [sqrt(1/2), sqrt(2)); log m = 2 atanh((m-1)/(m+1)).
+__device__ __forceinline__ double log_(double x) {
+  constexpr double LN2_HI = 0x1.62e42fee00000p-1;
+  constexpr double LN2_LO = 0x1.a39ef35793c76p-33;
+  const long long bits = __double_as_longlong(x);
+  int e = (int)((bits >> 52) & 0x7ff) - 1022;  // frexp exponent: x = m 2^e, m in [0.5, 1)
+  double m = __longlong_as_double((bits & 0x800fffffffffffffLL) | 0x3fe0000000000000LL);
+  if (m < 0.70710678118654752) {
+    m = 2.0 * m;
+    e -= 1;
+  }
+  const double s = (m - 1.0) / (m + 1.0);
+  const double z = s * s;
+  double p = 1.0 / 23.0;
+  p = fma_(p, z, 1.0 / 21.0);
+  p = fma_(p, z, 1.0 / 19.0);
+  p = fma_(p, z, 1.0 / 17.0);
+  p = fma_(p, z, 1.0 / 15.0);
+  p = fma_(p, z, 1.0 / 13.0);
+  p = fma_(p, z, 1.0 / 11.0);
+  p = fma_(p, z, 1.0 / 9.0);
+  p = fma_(p, z, 1.0 / 7.0);
+  p = fma_(p, z, 1.0 / 5.0);
+  p = fma_(p, z, 1.0 / 3.0);
+  p = fma_(p, z, 1.0);
+  const double t = (2.0 * s) * p;
+  const double ed = (double)e;
+  return fma_(ed, LN2_HI, fma_(ed, LN2_LO, t));
+}
+
+__device__ __forceinline__ bool finite_(double x) {
+  return (__double_as_longlong(x) & 0x7ff0000000000000LL) != 0x7ff0000000000000LL;
+}
+
+}  // namespace bz

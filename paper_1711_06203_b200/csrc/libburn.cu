@@ -1,0 +1,358 @@
+// libburn.cu -- the C ABI of include/burnzones.h: validation, table flattening, launches.
+// Host code is compiled with -ffp-contract=off; device code with -fmad=false.
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/burnzones.h"
+#include "bz_coop_main.cuh"
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+inline bool cuda_ok(cudaError_t e) {
+  if (e != cudaSuccess) {
+    g_last_cuda_error = (int)e;
+    return false;
+  }
+  return true;
+}
+#define BZ_CUDA(call)                      \
+  do {                                     \
+    if (!cuda_ok((call))) return BZ_ERR_CUDA; \
+  } while (0)
+
+// ln(x) for net_create (x = rate_A > 0, normal): same recipe as the device log_
+double host_log(double x) {
+  const double LN2_HI = 0x1.62e42fee00000p-1, LN2_LO = 0x1.a39ef35793c76p-33;
+  int e;
+  double m = std::frexp(x, &e);
+  if (m < 0.70710678118654752) {
+    m = 2.0 * m;
+    e -= 1;
+  }
+  const double s = (m - 1.0) / (m + 1.0);
+  const double z = s * s;
+  double p = 1.0 / 23.0;
+  for (int k = 10; k >= 0; k--) p = std::fma(p, z, 1.0 / (double)(2 * k + 1));
+  const double t = (2.0 * s) * p;
+  const double ed = (double)e;
+  return std::fma(ed, LN2_HI, std::fma(ed, LN2_LO, t));
+}
+
+typedef void (*KernelFn)(bz::DevNet, bz::BurnArgs);
+
+struct Variant {
+  const char *name;
+  int neq, lanes;
+  KernelFn fn;
+};
+
+#define BZ_VARIANT(NEQ, LANES) \
+  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, (KernelFn)bz::burn_coop_kernel<NEQ, LANES> }
+
+const Variant kVariants[] = {
+    BZ_VARIANT(3, 4),   BZ_VARIANT(4, 4),   BZ_VARIANT(8, 8),   BZ_VARIANT(14, 16),
+    BZ_VARIANT(16, 16), BZ_VARIANT(31, 32), BZ_VARIANT(32, 32),
+};
+
+const Variant *pick_variant(int n) {
+  if (n == 3) return &kVariants[0];
+  if (n <= 4) return &kVariants[1];
+  if (n <= 8) return &kVariants[2];
+  if (n == 14) return &kVariants[3];
+  if (n <= 16) return &kVariants[4];
+  if (n == 31) return &kVariants[5];
+  return &kVariants[6];
+}
+
+}  // namespace
+
+struct bz_net {
+  int N, n, K;
+  bz::DevNet dev;
+  double *d_dbl;
+  int *d_int;
+  unsigned long long *d_scratch;  // [0] queue head, [1..8] counters
+  const Variant *variant;
+  int grid, smem_bytes;
+  // staging for burn_zones_host
+  double *st_in, *st_out;
+  int32_t *st_nsteps;
+  int64_t st_cap;
+};
+
+extern "C" {
+
+int bz_last_cuda_error(void) { return g_last_cuda_error; }
+
+int net_create(const bz_net_desc *d, bz_net **out) {
+  if (!d || !out) return BZ_ERR_NULL;
+  *out = nullptr;
+  if (d->nspec < 1 || d->nspec > 31 || d->nreac < 1 || d->nreac > 256) return BZ_ERR_SIZE;
+  if (!d->aion || !d->reactant || !d->stoich_id || !d->stoich_dy || !d->rate_A || !d->rate_n ||
+      !d->rate_B || !d->q_mev)
+    return BZ_ERR_NULL;
+  const int N = d->nspec, K = d->nreac, n = N + 1;
+  if (!(d->cv > 0.0) || !std::isfinite(d->cv)) return BZ_ERR_NETWORK;
+  for (int i = 0; i < N; i++)
+    if (!(d->aion[i] > 0.0) || !std::isfinite(d->aion[i])) return BZ_ERR_NETWORK;
+
+  // ---- flatten -------------------------------------------------------------------------------
+  std::vector<int> rp(4 * K, 0);
+  std::vector<double> lnA(K), invsym(K);
+  std::vector<std::vector<std::pair<int, double>>> sp(N);  // species -> (k, dy), k ascending
+  std::vector<std::vector<int>> cl(N);                     // species -> (k | slot << 16)
+  for (int k = 0; k < K; k++) {
+    int r[3], m = 0;
+    for (int a = 0; a < 3; a++) {
+      const int id = d->reactant[3 * k + a];
+      if (id < 0) continue;
+      if (id >= N) return BZ_ERR_NETWORK;
+      r[m++] = id;
+    }
+    if (m == 0) return BZ_ERR_NETWORK;
+    if (!(d->rate_A[k] > 0.0) || !std::isfinite(d->rate_A[k]) || !std::isfinite(d->rate_n[k]) ||
+        !std::isfinite(d->rate_B[k]) || !std::isfinite(d->q_mev[k]))
+      return BZ_ERR_NETWORK;
+    // distinct reactant species in order of first appearance = Jacobian column slots
+    int col[3] = {0, 0, 0}, nslot = 0;
+    for (int a = 0; a < m; a++) {
+      bool seen = false;
+      for (int b = 0; b < a; b++) seen |= (r[b] == r[a]);
+      if (!seen) col[nslot++] = r[a];
+    }
+    const int same = (m > 1 && r[0] == r[1]) + (m > 2 && r[0] == r[2]) + (m > 2 && r[1] == r[2]);
+    invsym[k] = same == 0 ? 1.0 : (same == 1 ? 0.5 : 1.0 / 6.0);
+    lnA[k] = host_log(d->rate_A[k]);
+    rp[4 * k + 0] = m | (nslot << 8);
+    rp[4 * k + 1] = r[0] | ((m > 1 ? r[1] : 0) << 8) | ((m > 2 ? r[2] : 0) << 16);
+    rp[4 * k + 2] = col[0] | (col[1] << 8) | (col[2] << 16);
+    for (int s = 0; s < nslot; s++) cl[col[s]].push_back(k | (s << 16));
+    int ids[4], nid = 0;
+    for (int a = 0; a < 4; a++) {
+      const int id = d->stoich_id[4 * k + a];
+      if (id < 0) continue;
+      if (id >= N) return BZ_ERR_NETWORK;
+      for (int b = 0; b < nid; b++)
+        if (ids[b] == id) return BZ_ERR_NETWORK;
+      if (!std::isfinite(d->stoich_dy[4 * k + a])) return BZ_ERR_NETWORK;
+      ids[nid++] = id;
+      sp[id].push_back({k, d->stoich_dy[4 * k + a]});
+    }
+  }
+  std::vector<int> sp_off(N + 1, 0), sp_k, cl_off(N + 1, 0), cl_ks;
+  std::vector<double> sp_dy;
+  for (int i = 0; i < N; i++) {
+    for (auto &t : sp[i]) {
+      sp_k.push_back(t.first);
+      sp_dy.push_back(t.second);
+    }
+    sp_off[i + 1] = (int)sp_k.size();
+    for (int c : cl[i]) cl_ks.push_back(c);
+    cl_off[i + 1] = (int)cl_ks.size();
+  }
+  const int nterm = (int)sp_k.size(), ncl = (int)cl_ks.size();
+  std::vector<double> dbl;
+  dbl.insert(dbl.end(), lnA.begin(), lnA.end());
+  dbl.insert(dbl.end(), d->rate_n, d->rate_n + K);
+  dbl.insert(dbl.end(), d->rate_B, d->rate_B + K);
+  dbl.insert(dbl.end(), d->q_mev, d->q_mev + K);
+  dbl.insert(dbl.end(), invsym.begin(), invsym.end());
+  dbl.insert(dbl.end(), d->aion, d->aion + N);
+  dbl.insert(dbl.end(), sp_dy.begin(), sp_dy.end());
+  std::vector<int> itab;
+  itab.insert(itab.end(), rp.begin(), rp.end());
+  itab.insert(itab.end(), sp_off.begin(), sp_off.end());
+  itab.insert(itab.end(), sp_k.begin(), sp_k.end());
+  itab.insert(itab.end(), cl_off.begin(), cl_off.end());
+  itab.insert(itab.end(), cl_ks.begin(), cl_ks.end());
+
+  bz_net *h = new (std::nothrow) bz_net();
+  if (!h) return BZ_ERR_NOMEM;
+  std::memset(h, 0, sizeof(*h));
+  h->N = N; h->n = n; h->K = K;
+  h->variant = pick_variant(n);
+
+  // ---- upload --------------------------------------------------------------------------------
+  auto fail = [&](int code) {
+    net_destroy(h);
+    return code;
+  };
+  if (!cuda_ok(cudaMalloc(&h->d_dbl, dbl.size() * sizeof(double)))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMalloc(&h->d_int, itab.size() * sizeof(int)))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMalloc(&h->d_scratch, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMemcpy(h->d_dbl, dbl.data(), dbl.size() * sizeof(double), cudaMemcpyHostToDevice)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMemcpy(h->d_int, itab.data(), itab.size() * sizeof(int), cudaMemcpyHostToDevice)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMemset(h->d_scratch, 0, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
+  h->dev.N = N; h->dev.n = n; h->dev.K = K; h->dev.nterm = nterm; h->dev.ncl = ncl;
+  h->dev.fac = 9.648533212331e17 / d->cv;
+  h->dev.dbl = h->d_dbl; h->dev.itab = h->d_int;
+  h->dev.ndbl = (int)dbl.size(); h->dev.nint = (int)itab.size();
+
+  // ---- launch geometry: persistent grid, blocks/SM from the occupancy calculator -----------------
+  const int L = h->variant->lanes;
+  const int gpb = bz::COOP_THREADS / L;
+  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
+  const int tab = ((h->dev.ndbl + 1) & ~1) + (((h->dev.nint + 3) & ~3) / 2);
+  h->smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
+  int dev = 0, sms = 0, bps = 0;
+  if (!cuda_ok(cudaGetDevice(&dev))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaFuncSetAttribute((const void *)h->variant->fn,
+                                    cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->variant->fn,
+                                                             bz::COOP_THREADS, h->smem_bytes)))
+    return fail(BZ_ERR_CUDA);
+  if (bps < 1) return fail(BZ_ERR_NOMEM);
+  h->grid = sms * bps;
+  *out = h;
+  return BZ_OK;
+}
+
+int net_destroy(bz_net *h) {
+  if (!h) return BZ_ERR_NULL;
+  if (h->d_dbl) cudaFree(h->d_dbl);
+  if (h->d_int) cudaFree(h->d_int);
+  if (h->d_scratch) cudaFree(h->d_scratch);
+  if (h->st_in) cudaFree(h->st_in);
+  if (h->st_out) cudaFree(h->st_out);
+  if (h->st_nsteps) cudaFree(h->st_nsteps);
+  delete h;
+  return BZ_OK;
+}
+
+int bz_norm_lanes(const bz_net *h) { return h ? h->variant->lanes : BZ_ERR_NULL; }
+const char *bz_kernel_name(const bz_net *h) { return h ? h->variant->name : ""; }
+
+int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+               double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
+               void *cuda_stream) {
+  if (!h) return BZ_ERR_NULL;
+  if (nz < 0) return BZ_ERR_SIZE;
+  if (!(dt > 0.0) || !(rtol > 0.0) || !(atol >= 0.0) || !std::isfinite(dt) || !std::isfinite(rtol) ||
+      !std::isfinite(atol))
+    return BZ_ERR_SCALAR;
+  if (nz == 0) return BZ_OK;
+  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  BZ_CUDA(cudaMemsetAsync(h->d_scratch, 0, 16 * sizeof(unsigned long long), st));
+  bz::BurnArgs a;
+  a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
+  a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
+  a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
+  const int L = h->variant->lanes;
+  const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
+  const int grid = (int)(groups_needed < h->grid ? groups_needed : h->grid);
+  void *args[] = {(void *)&h->dev, (void *)&a};
+  BZ_CUDA(cudaLaunchKernel((const void *)h->variant->fn, dim3(grid), dim3(bz::COOP_THREADS), args,
+                           (size_t)h->smem_bytes, st));
+  return BZ_OK;
+}
+
+int bz_get_counters(const bz_net *h, void *cuda_stream, uint64_t out[8]) {
+  if (!h || !out) return BZ_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned long long tmp[8];
+  BZ_CUDA(cudaMemcpyAsync(tmp, h->d_scratch + 1, sizeof(tmp), cudaMemcpyDeviceToHost, st));
+  BZ_CUDA(cudaStreamSynchronize(st));
+  for (int i = 0; i < 8; i++) out[i] = tmp[i];
+  return BZ_OK;
+}
+
+int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+                    double dt, double rtol, double atol, double *T_out, double *X_out,
+                    int32_t *nsteps, void *cuda_stream) {
+  if (!h) return BZ_ERR_NULL;
+  if (nz < 0) return BZ_ERR_SIZE;
+  if (nz == 0) return BZ_OK;
+  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int N = h->N;
+  if (h->st_cap < nz) {
+    BZ_CUDA(cudaStreamSynchronize(st));
+    if (h->st_in) cudaFree(h->st_in);
+    if (h->st_out) cudaFree(h->st_out);
+    if (h->st_nsteps) cudaFree(h->st_nsteps);
+    h->st_in = h->st_out = nullptr;
+    h->st_nsteps = nullptr;
+    h->st_cap = 0;
+    if (!cuda_ok(cudaMalloc(&h->st_in, (size_t)(N + 2) * nz * sizeof(double)))) return BZ_ERR_NOMEM;
+    if (!cuda_ok(cudaMalloc(&h->st_out, (size_t)(N + 1) * nz * sizeof(double)))) return BZ_ERR_NOMEM;
+    if (!cuda_ok(cudaMalloc(&h->st_nsteps, (size_t)nz * sizeof(int32_t)))) return BZ_ERR_NOMEM;
+    h->st_cap = nz;
+  }
+  double *d_rho = h->st_in, *d_T = h->st_in + nz, *d_X = h->st_in + 2 * nz;
+  double *d_To = h->st_out, *d_Xo = h->st_out + nz;
+  BZ_CUDA(cudaMemcpyAsync(d_rho, rho, nz * sizeof(double), cudaMemcpyHostToDevice, st));
+  BZ_CUDA(cudaMemcpyAsync(d_T, T, nz * sizeof(double), cudaMemcpyHostToDevice, st));
+  BZ_CUDA(cudaMemcpyAsync(d_X, X, (size_t)N * nz * sizeof(double), cudaMemcpyHostToDevice, st));
+  int rc = burn_zones(h, nz, d_rho, d_T, d_X, dt, rtol, atol, d_To, d_Xo, h->st_nsteps, cuda_stream);
+  if (rc != BZ_OK) return rc;
+  BZ_CUDA(cudaMemcpyAsync(T_out, d_To, nz * sizeof(double), cudaMemcpyDeviceToHost, st));
+  BZ_CUDA(cudaMemcpyAsync(X_out, d_Xo, (size_t)N * nz * sizeof(double), cudaMemcpyDeviceToHost, st));
+  BZ_CUDA(cudaMemcpyAsync(nsteps, h->st_nsteps, nz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  return BZ_OK;
+}
+
+}  // extern "C"
+
+// ---- FP64 peak probe ----------------------------------------------------------------------------
+namespace {
+__global__ void __launch_bounds__(256) dfma_probe_kernel(long long iters, double *sink) {
+  double a[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) a[i] = 1.0 + 1e-9 * (threadIdx.x + i);
+  const double m = 1.0000000001, c = 1e-12;
+  for (long long it = 0; it < iters; it++) {
+#pragma unroll
+    for (int r = 0; r < 32; r++) {
+#pragma unroll
+      for (int i = 0; i < 8; i++) a[i] = __fma_rn(a[i], m, c);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; i++) s += a[i];
+  if (s == 123.456) sink[0] = s;
+}
+}  // namespace
+
+extern "C" int bz_fp64_peak_probe(int64_t iters, void *cuda_stream, double *tflops, double *ms) {
+  if (!tflops || !ms) return BZ_ERR_NULL;
+  if (iters < 1) return BZ_ERR_SIZE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  BZ_CUDA(cudaGetDevice(&dev));
+  BZ_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  double *sink = nullptr;
+  BZ_CUDA(cudaMalloc(&sink, sizeof(double)));
+  cudaEvent_t e0, e1;
+  BZ_CUDA(cudaEventCreate(&e0));
+  BZ_CUDA(cudaEventCreate(&e1));
+  const int blocks = sms * 8, threads = 256;
+  dfma_probe_kernel<<<blocks, threads, 0, st>>>(iters / 8 + 1, sink);  // warm-up
+  BZ_CUDA(cudaEventRecord(e0, st));
+  dfma_probe_kernel<<<blocks, threads, 0, st>>>(iters, sink);
+  BZ_CUDA(cudaEventRecord(e1, st));
+  BZ_CUDA(cudaEventSynchronize(e1));
+  float t = 0.f;
+  BZ_CUDA(cudaEventElapsedTime(&t, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  const double flops = 2.0 * 8.0 * 32.0 * (double)iters * (double)blocks * (double)threads;
+  *ms = (double)t;
+  *tflops = flops / ((double)t * 1e-3) / 1e12;
+  return BZ_OK;
+}

@@ -1,0 +1,134 @@
+"""GPU parity: burn_zones (through the C ABI) against the CPU oracle on the same seeded inputs.
+Bar (BASELINE.json north_star): rel. error <= 1e-5 on final X > 1e-10, <= 1e-6 on final T,
+at rtol = 1e-8.  Under the determinism contract the expected outcome is
+bit-identical X, T and nsteps; the tests report how close to that the run was."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload, network_for_config, first_order_decay_network
+from _parity import compare
+
+pytestmark = pytest.mark.gpu
+
+OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+def _gpu_burn(w, rho=None, T=None, X=None):
+    import torch
+    import paper_1711_06203_b200 as bz
+    net = bz.net_create(w.net)
+    dev = torch.device("cuda:0")
+    rho_d = torch.from_numpy(w.rho if rho is None else rho).to(dev)
+    T_d = torch.from_numpy(w.T if T is None else T).to(dev)
+    X_d = torch.from_numpy(w.X if X is None else X).to(dev)
+    To, Xo, ns = bz.burn_zones(net, rho_d, T_d, X_d, w.dt, w.rtol, w.atol)
+    torch.cuda.synchronize()
+    cnt = bz.get_counters(net)
+    lanes, name = net.norm_lanes, net.kernel_name
+    out = To.cpu().numpy(), Xo.cpu().numpy(), ns.cpu().numpy(), cnt, lanes, name
+    bz.net_destroy(net)
+    return out
+
+
+def _record(tag, stats):
+    os.makedirs(OUT, exist_ok=True)
+    with open(os.path.join(OUT, "parity_stats.jsonl"), "a") as fh:
+        fh.write(json.dumps(dict(tag=tag, **stats)) + "\n")
+
+
+# sizes: several tiles (blocks x groups) and a ragged tail; the oracle finishes in seconds
+@pytest.mark.parametrize("config,zones", [(1, None), (2, 61), (3, 509), (5, 4099)])
+def test_parity_sampled_configs(config, zones):
+    w = make_workload(config, zones=zones)
+    To, Xo, ns, cnt, lanes, name = _gpu_burn(w)
+    Tr, Xr, nr, cr = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=lanes)
+    stats = compare(To, Xo, ns, Tr, Xr, nr)
+    stats.update(kernel=name, counters_equal=all(cnt[k] == cr[k] for k in cnt))
+    _record(f"config{config}", stats)
+    assert stats["nsteps_equal"] > 0.99
+    # mass invariant on the GPU result itself (north_star: 1e-10)
+    ok = ns > 0
+    assert np.abs(Xo.sum(axis=0) - w.X.sum(axis=0))[ok].max() <= 1e-10
+
+
+def test_parity_config4_hotspot_and_cold():
+    """Divergence stress: an x-y slab through a hotspot centre (steps 1 ... ~400 side by side)
+    plus a strided cold sample."""
+    c = make_workload(4, zones=[0]).meta["centres"][0].astype(int)
+    ii, jj = np.meshgrid(np.arange(max(c[0] - 20, 0), min(c[0] + 20, 256)),
+                         np.arange(max(c[1] - 6, 0), min(c[1] + 6, 256)), indexing="ij")
+    slab = (ii + 256 * (jj + 256 * c[2])).ravel()
+    zones = np.unique(np.concatenate([slab, np.arange(0, 256 ** 3, 16411)]))
+    w = make_workload(4, zones=zones)
+    To, Xo, ns, cnt, lanes, name = _gpu_burn(w)
+    Tr, Xr, nr, cr = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=lanes)
+    stats = compare(To, Xo, ns, Tr, Xr, nr)
+    _record("config4", dict(stats, kernel=name))
+    assert nr.min() == 1 and nr.max() > 100
+
+
+def test_closed_form_on_gpu():
+    """The closed-form pin of north_star evaluated on the CUDA path directly."""
+    import math
+    lamdt = 5.0
+    net = first_order_decay_network(lamdt / 1e-6)
+    w = make_workload(1, zones=[0])
+    w.net, w.dt = net, 1e-6
+    X = np.array([[0.7], [0.1]])
+    To, Xo, ns, *_ = _gpu_burn(w, rho=np.array([1e6]), T=np.array([2e9]), X=X)
+    assert To[0] == 2e9 and ns[0] > 0
+    ref = 0.7 / 4 * math.exp(-lamdt)
+    assert abs(Xo[0, 0] / 4 - ref) <= 100 * (1e-8 * ref + 1e-12)
+
+
+def test_edge_cases():
+    import torch
+    import paper_1711_06203_b200 as bz
+    net_d = network_for_config(1)
+    net = bz.net_create(net_d)
+    dev = torch.device("cuda:0")
+    # nz = 0 is a no-op
+    e = torch.empty(0, dtype=torch.float64, device=dev)
+    bz.burn_zones(net, e, e, torch.empty((2, 0), dtype=torch.float64, device=dev), 1e-6, 1e-8, 1e-12)
+    # invalid zones get -4 and keep their inputs; valid neighbours are unaffected
+    rho = np.array([1e8, -1.0, 1e8, 1e8, np.nan, 3e7, 3e7])
+    T = np.array([2e9, 2e9, 0.0, np.inf, 2e9, 2.5e9, 3e8])
+    X = np.array([[0.4] * 7, [0.0] * 7])
+    To, Xo, ns = bz.burn_zones(net, torch.from_numpy(rho).to(dev), torch.from_numpy(T).to(dev),
+                               torch.from_numpy(X).to(dev), 1e-6, 1e-8, 1e-12)
+    torch.cuda.synchronize()
+    Tr, Xr, nr, _ = oracle.burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, norm_lanes=net.norm_lanes)
+    assert list(ns.cpu().numpy()[1:5]) == [-4] * 4
+    assert np.array_equal(ns.cpu().numpy(), nr)
+    assert np.array_equal(Xo.cpu().numpy()[:, [0, 5, 6]], Xr[:, [0, 5, 6]])
+    assert np.array_equal(Xo.cpu().numpy()[:, 1:5], X[:, 1:5])
+    # exact aliasing of inputs and outputs is allowed
+    r_d, T_d, X_d = (torch.from_numpy(a).to(dev) for a in (rho, T, X))
+    bz.burn_zones(net, r_d, T_d, X_d, 1e-6, 1e-8, 1e-12, T_out=T_d, X_out=X_d)
+    torch.cuda.synchronize()
+    assert np.array_equal(X_d.cpu().numpy()[:, [0, 5, 6]], Xr[:, [0, 5, 6]])
+    # bad scalars are call-level errors
+    with pytest.raises(bz.BurnError) as ei:
+        bz.burn_zones(net, r_d, T_d, X_d, -1.0, 1e-8, 1e-12)
+    assert ei.value.code == -4
+    bz.net_destroy(net)
+
+
+def test_host_path_matches_device_path():
+    import torch
+    import paper_1711_06203_b200 as bz
+    w = make_workload(1)
+    net = bz.net_create(w.net)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    To = torch.empty(w.nz, dtype=torch.float64).pin_memory()
+    Xo = torch.empty((2, w.nz), dtype=torch.float64).pin_memory()
+    ns = torch.empty(w.nz, dtype=torch.int32).pin_memory()
+    bz.burn_zones_host(net, pin(w.rho), pin(w.T), pin(w.X), w.dt, w.rtol, w.atol, To, Xo, ns)
+    torch.cuda.synchronize()
+    Td, Xd, nd, *_ = _gpu_burn(w)
+    assert np.array_equal(To.numpy(), Td) and np.array_equal(Xo.numpy(), Xd) and np.array_equal(ns.numpy(), nd)
+    bz.net_destroy(net)
