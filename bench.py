@@ -1,0 +1,256 @@
+#!/usr/bin/env python
+"""bench.py -- zones burned/sec on the 13-isotope 128^3 config (BASELINE.json configs[2]).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+
+A "step" is one pass of the whole hot path (a1-a9: load, work queue, rates, Jacobian, LU,
+Newton, BDF control, store) over one batch of synthetic zones: one burn_zones call.
+N > 1: one process per GPU (torchrun), every rank burns its own copy of the config (weak
+scaling, no data-path collective); value = zones of all ranks / max time.
+Prints ONE JSON line on rank 0.  DESIGN.md section 6 defines every field.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import CONFIG_NZ, make_workload  # noqa: E402
+
+METRIC = "zones burned/sec (13-isotope net, fp64 BDF)"
+UNIT = "zones/s"
+FP64_LANES_PER_SM = 64           # DFMA lanes per SM
+CPU_SAMPLE_STRIDE = {1: 1, 2: 16, 3: 64, 4: 64, 5: 512}
+
+
+def _workload_name(cfg):
+    return {1: "config1 carbon 3-ODE 4096 zones", 2: "config2 alpha7 64^3", 3: "config3 alpha13 128^3 XRB-like",
+            4: "config4 alpha13 256^3 hotspots", 5: "config5 synth30 128^3"}[cfg]
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows = []
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.gpu)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 9 for n, v in zip(names, r[5:9]) if v.lower().startswith("active")})
+        pw = [float(r[3]) for r in self.rows if len(r) >= 9 and r[3].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores, on a bounded sample of the
+    same workload (every s-th zone).  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    stride = CPU_SAMPLE_STRIDE[args.config]
+    w = make_workload(args.config, zones=stride if stride > 1 else None)
+    cores = oracle.max_threads()
+    for _ in range(args.warmup):
+        oracle.burn(w.net, w.rho[:256], w.T[:256], w.X[:, :256], w.dt, w.rtol, w.atol)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol)
+    el = (time.perf_counter() - t0) / args.steps
+    value = w.nz / el
+    sample = f"every {stride}th zone of {_workload_name(args.config)} ({w.nz} zones per step)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": el * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": _workload_name(args.config), "zones_per_step": w.nz, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1711_06203_b200 as bz
+    from paper_1711_06203_b200.flops import algorithmic_flops, flop_model, state_bytes_per_zone
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the burn has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = args.config
+    w = make_workload(cfg)                       # every rank burns its own full copy (weak scaling)
+    nz, N = w.nz, w.net.nspec
+    net = bz.net_create(w.net)
+    stream = torch.cuda.current_stream()
+
+    # ---- device-resident arm -------------------------------------------------------------------
+    rho_d, T_d, X_d = (torch.from_numpy(a).to(dev) for a in (w.rho, w.T, w.X))
+    To_d, Xo_d = torch.empty_like(T_d), torch.empty_like(X_d)
+    ns_d = torch.empty(nz, dtype=torch.int32, device=dev)
+
+    def step():
+        bz.burn_zones(net, rho_d, T_d, X_d, w.dt, w.rtol, w.atol, T_out=To_d, X_out=Xo_d, nsteps=ns_d, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record(stream)
+    for i in range(args.steps):
+        step()
+        ev[i + 1].record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[-1])
+    counters = bz.get_counters(net)              # of the last launch
+    nfail = int((ns_d < 0).sum().item())
+
+    # ---- end-to-end arm: host buffers through the C ABI, copies inside the timed region --------
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    rho_h, T_h, X_h = pin(w.rho), pin(w.T), pin(w.X)
+    To_h = torch.empty(nz, dtype=torch.float64).pin_memory()
+    Xo_h = torch.empty((N, nz), dtype=torch.float64).pin_memory()
+    ns_h = torch.empty(nz, dtype=torch.int32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    bz.burn_zones_host(net, rho_h, T_h, X_h, w.dt, w.rtol, w.atol, To_h, Xo_h, ns_h, stream=stream)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        bz.burn_zones_host(net, rho_h, T_h, X_h, w.dt, w.rtol, w.atol, To_h, Xo_h, ns_h, stream=stream)
+    e1.record(stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / e2e_steps
+    same = bool(np.array_equal(Xo_h.numpy(), Xo_d.cpu().numpy()))
+
+    # ---- max over ranks ------------------------------------------------------------------------
+    tms = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(tms[0]), float(tms[1])
+    ms_per_step = total_ms / args.steps
+    value = world * nz / (ms_per_step * 1e-3)
+    e2e_value = world * nz / (e2e_ms * 1e-3)
+
+    if rank == 0:
+        # roofline of the dominant (only) kernel: plain FP64 ALUs
+        props = torch.cuda.get_device_properties(dev)
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+        peak_tf = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+        probe_tf, _ = bz.fp64_peak_probe(20000)
+        aflops = algorithmic_flops(w.net, counters)
+        kern_ms = float(np.mean(per_launch_ms))
+        achieved = aflops / (kern_ms * 1e-3) / 1e12
+        sbytes = state_bytes_per_zone(N)
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")      # written from an ncu --set full capture
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get(f"config{cfg}:{net.kernel_name}")
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": _workload_name(cfg), "zones_per_gpu": nz, "neq": N + 1, "nreac": w.net.nreac,
+                       "dt": w.dt, "rtol": w.rtol, "atol": w.atol, "kernel": net.kernel_name,
+                       "l2": f"inputs {8 * (N + 2) * nz / 1e6:.0f} MB per step exceed the 126 MB L2",
+                       "parallelism": f"zones sharded, {world} replica(s), no collective"},
+            "rhs_evals_per_s": world * counters["nrhs"] / (kern_ms * 1e-3),
+            "steps_per_zone_mean": counters["nst"] / nz, "failed_zones": nfail, "counters": counters,
+            "hbm_state_gbs": sbytes * nz / (kern_ms * 1e-3) / 1e9,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": achieved / peak_tf, "traffic": traffic,
+                         "peak_source": f"{props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
+                                        f"{sm_max_mhz:.0f} MHz (derived); DFMA probe measured {probe_tf:.2f} TFLOP/s",
+                         "frac_of_measured_probe": achieved / probe_tf,
+                         "algorithmic_flops_per_launch": aflops, "kernel_ms": kern_ms,
+                         "flop_model": flop_model(w.net)},
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": 8 * (N + 2) * nz, "d2h_bytes_per_step": (8 * (N + 1) + 4) * nz,
+                    "matches_device_path": same},
+            "gpu_launches": args.steps, "clocks": clocks,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            import oracle
+            stride = CPU_SAMPLE_STRIDE[cfg]
+            ws = make_workload(cfg, zones=stride if stride > 1 else None)
+            t0 = time.perf_counter()
+            oracle.burn(ws.net, ws.rho, ws.T, ws.X, ws.dt, ws.rtol, ws.atol)
+            el = time.perf_counter() - t0
+            out["cpu_baseline"] = {"value": ws.nz / el, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+                                   "sample": f"every {stride}th zone ({ws.nz} zones), {el:.1f} s wall"}
+        print(json.dumps(out))
+    bz.net_destroy(net)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
