@@ -152,6 +152,11 @@ static int net_init(Net *nt, const orc_net_desc *d) {
  * ~atol) do not feed the rate products, which would otherwise be unstable (reading s19).
  * Accumulation order: reactions k ascending; per reaction the stoichiometry entries in table
  * order; the temperature row accumulates sum_k Q_k (.) and is scaled by fac at the end. */
+/* Internal ordering of the unknowns (reading s25): y = (T, Y_0, ..., Y_{N-1}),
+ * temperature FIRST.  The temperature equation carries the largest Jacobian entries
+ * (N_A MeV/c_v ~ 1e10), so with T first partial pivoting keeps the natural order. */
+#define SP(i) ((i) + 1)
+#define TI 0
 static void rates(const Net *nt, double rho, const double *y, double *f, double *J) {
   const int N = nt->N, n = nt->n;
   double sT = 0.0, JT[ORC_NMAX], ya[ORC_NMAX];
@@ -160,8 +165,8 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
     for (int i = 0; i < n * n; i++) J[i] = 0.0;
     for (int j = 0; j < n; j++) JT[j] = 0.0;
   }
-  for (int i = 0; i < N; i++) ya[i] = fabs(y[i]);
-  const double T = y[N];
+  for (int i = 0; i < N; i++) ya[i] = fabs(y[SP(i)]);
+  const double T = y[TI];
   const double T9 = T * 1e-9;
   const double lnT9 = orc_log(T9);
   const double t13 = orc_exp(lnT9 * (-1.0 / 3.0));
@@ -175,11 +180,11 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
     double lam = orc_exp(arg);
     double pref = (lam * rhopow[m]) * nt->invsym[k];
     int anyneg = 0;
-    for (int a = 0; a < m; a++) anyneg |= (y[r[a]] < 0.0);
+    for (int a = 0; a < m; a++) anyneg |= (y[SP(r[a])] < 0.0);
     double R = pref;
     for (int a = 0; a < m; a++) R = R * ya[r[a]];
     if (anyneg) R = -R; /* reading s19: odd, monotone extension to Y < 0 */
-    for (int s = 0; s < nt->ns[k]; s++) f[nt->sid[k][s]] = fma(nt->sdy[k][s], R, f[nt->sid[k][s]]);
+    for (int s = 0; s < nt->ns[k]; s++) f[SP(nt->sid[k][s])] = fma(nt->sdy[k][s], R, f[SP(nt->sid[k][s])]);
     sT = fma(nt->Q[k], R, sT);
     if (!J) continue;
     /* species columns: distinct reactant species in order of first appearance */
@@ -202,25 +207,25 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
         first = 0;
       }
       double dRdY = (m == 1) ? pref : pref * d;
-      if (anyneg && !(y[j] < 0.0)) dRdY = -dRdY;
+      if (anyneg && !(y[SP(j)] < 0.0)) dRdY = -dRdY;
       for (int s = 0; s < nt->ns[k]; s++) {
-        int i = nt->sid[k][s];
-        J[i * n + j] = fma(nt->sdy[k][s], dRdY, J[i * n + j]);
+        int i = SP(nt->sid[k][s]);
+        J[i * n + SP(j)] = fma(nt->sdy[k][s], dRdY, J[i * n + SP(j)]);
       }
-      JT[j] = fma(nt->Q[k], dRdY, JT[j]);
+      JT[SP(j)] = fma(nt->Q[k], dRdY, JT[SP(j)]);
     }
     /* temperature column */
     double g = fma(nt->B[k], t13third, nt->en[k]);
     double dRdT = (R * g) * invT;
     for (int s = 0; s < nt->ns[k]; s++) {
-      int i = nt->sid[k][s];
-      J[i * n + N] = fma(nt->sdy[k][s], dRdT, J[i * n + N]);
+      int i = SP(nt->sid[k][s]);
+      J[i * n + TI] = fma(nt->sdy[k][s], dRdT, J[i * n + TI]);
     }
-    JT[N] = fma(nt->Q[k], dRdT, JT[N]);
+    JT[TI] = fma(nt->Q[k], dRdT, JT[TI]);
   }
-  f[N] = nt->fac * sT;
+  f[TI] = nt->fac * sT;
   if (J)
-    for (int j = 0; j < n; j++) J[N * n + j] = nt->fac * JT[j];
+    for (int j = 0; j < n; j++) J[TI * n + j] = nt->fac * JT[j];
 }
 
 /* ---- dense LU, LINPACK dgefa/dgesl order (step a5/a6; C.5 item 4) ------------------- */
@@ -337,7 +342,8 @@ static double eta_of(double E, double bias, int p) {
 static int invalid_state(int n, const double *y) {
   for (int i = 0; i < n; i++)
     if (!isfinite(y[i])) return 1;
-  return !(y[n - 1] > 0.0);
+  (void)n;
+  return !(y[TI] > 0.0);
 }
 static void set_weights(int n, const double *y, double rtol, double atol, double *w) {
   for (int i = 0; i < n; i++) w[i] = 1.0 / fma(rtol, fabs(y[i]), atol);
@@ -402,7 +408,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
     h = o->fixed_h;
     q = o->fixed_q;
     for (int j = 0; j <= q; j++)
-      for (int i = 0; i < n; i++) Z[j][i] = o->z_init[j * n + i];
+      for (int i = 0; i < n; i++) Z[j][i] = o->z_init[j * n + (i == TI ? n - 1 : i - 1)]; /* API order: T last */
     for (int i = 1; i <= 5; i++) tau[i] = h;
     ntau = 5;
   }
@@ -654,7 +660,18 @@ int orc_rates(const orc_net_desc *d, double rho, const double *y, double *f, dou
   Net nt;
   int rc = net_init(&nt, d);
   if (rc) return rc;
-  rates(&nt, rho, y, f, J);
+  /* API order is (Y_0..Y_{N-1}, T); permute to the internal T-first order and back */
+  const int n = nt.n, N = nt.N;
+  double yi[ORC_NMAX], fi[ORC_NMAX], Ji[ORC_NMAX * ORC_NMAX];
+  int ext[ORC_NMAX]; /* internal index -> external index */
+  ext[TI] = N;
+  for (int i = 0; i < N; i++) ext[SP(i)] = i;
+  for (int a = 0; a < n; a++) yi[a] = y[ext[a]];
+  rates(&nt, rho, yi, fi, J ? Ji : NULL);
+  for (int a = 0; a < n; a++) f[ext[a]] = fi[a];
+  if (J)
+    for (int a = 0; a < n; a++)
+      for (int b = 0; b < n; b++) J[ext[a] * n + ext[b]] = Ji[a * n + b];
   return 0;
 }
 
@@ -682,15 +699,15 @@ int orc_burn(const orc_net_desc *d, int64_t nz, const double *rho, const double 
 #pragma omp for schedule(dynamic, 64)
     for (int64_t z = 0; z < nz; z++) {
       double y0[ORC_NMAX], yout[ORC_NMAX];
-      for (int i = 0; i < N; i++) y0[i] = X[(int64_t)i * nz + z] / nt.aion[i];
-      y0[N] = T[z];
+      for (int i = 0; i < N; i++) y0[SP(i)] = X[(int64_t)i * nz + z] / nt.aion[i];
+      y0[TI] = T[z];
       int code = burn_zone(&nt, rho[z], y0, dt, rtol, atol, opts, yout, cnt);
       if (code == -4) { /* invalid input: outputs = inputs */
         for (int i = 0; i < N; i++) X_out[(int64_t)i * nz + z] = X[(int64_t)i * nz + z];
         T_out[z] = T[z];
       } else {
-        for (int i = 0; i < N; i++) X_out[(int64_t)i * nz + z] = nt.aion[i] * yout[i];
-        T_out[z] = yout[N];
+        for (int i = 0; i < N; i++) X_out[(int64_t)i * nz + z] = nt.aion[i] * yout[SP(i)];
+        T_out[z] = yout[TI];
       }
       nsteps[z] = code;
       if (code < 0) cnt[7]++;

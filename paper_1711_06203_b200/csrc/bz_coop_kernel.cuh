@@ -63,7 +63,7 @@ struct Group {
     sync();  // previous readers of the scratch are done
     if (lig < n) ysh[lig] = y;
     sync();
-    const double T = ysh[N];
+    const double T = ysh[0];  // internal order: T first, species i at i + 1
     const double T9 = T * 1e-9;
     const double lnT9 = log_(T9);
     const double t13 = exp_(lnT9 * (-1.0 / 3.0));
@@ -77,7 +77,7 @@ struct Group {
       const double arg = fma_(-B[k], t13, fma_(en[k], lnT9, lnA[k]));
       const double lam = exp_(arg);
       const double pref = (lam * (m == 1 ? 1.0 : (m == 2 ? rho : rho2))) * invsym[k];
-      const double y0 = ysh[r0];
+      const double y0 = ysh[r0 + 1];
       const double v0 = fabs(y0);
       double Rk, d0, d1 = 0.0, d2 = 0.0;
       bool neg0 = y0 < 0.0, neg1 = false, neg2 = false;
@@ -85,7 +85,7 @@ struct Group {
         Rk = pref * v0;
         d0 = pref;
       } else if (m == 2) {
-        const double y1 = ysh[r1];
+        const double y1 = ysh[r1 + 1];
         const double v1 = fabs(y1);
         neg1 = y1 < 0.0;
         Rk = (pref * v0) * v1;
@@ -96,7 +96,7 @@ struct Group {
           d1 = pref * v0;
         }
       } else {
-        const double y1 = ysh[r1], y2 = ysh[r2];
+        const double y1 = ysh[r1 + 1], y2 = ysh[r2 + 1];
         const double v1 = fabs(y1), v2 = fabs(y2);
         neg1 = y1 < 0.0;
         neg2 = y2 < 0.0;
@@ -124,9 +124,9 @@ struct Group {
         const int c0 = rpk.z & 0xff, c1 = (rpk.z >> 8) & 0xff, c2 = (rpk.z >> 16) & 0xff;
         const int nslot = (rpk.x >> 8) & 0xff;
         if (anyneg) {
-          if (!(ysh[c0] < 0.0)) d0 = -d0;
-          if (nslot > 1 && !(ysh[c1] < 0.0)) d1 = -d1;
-          if (nslot > 2 && !(ysh[c2] < 0.0)) d2 = -d2;
+          if (!(ysh[c0 + 1] < 0.0)) d0 = -d0;
+          if (nslot > 1 && !(ysh[c1 + 1] < 0.0)) d1 = -d1;
+          if (nslot > 2 && !(ysh[c2 + 1] < 0.0)) d2 = -d2;
         }
         dRdY[3 * k + 0] = d0;
         dRdY[3 * k + 1] = d1;
@@ -137,10 +137,11 @@ struct Group {
     }
     sync();
     double f = 0.0;
-    if (lig < N) {
-      const int e = sp_off[lig + 1];
-      for (int t = sp_off[lig]; t < e; t++) f = fma_(sp_dy[t], R[sp_k[t]], f);
-    } else if (lig == N) {
+    const int sp = lig - 1;  // my species (lanes 1..N); lane 0 owns T
+    if (lig >= 1 && lig <= N) {
+      const int e = sp_off[sp + 1];
+      for (int t = sp_off[sp]; t < e; t++) f = fma_(sp_dy[t], R[sp_k[t]], f);
+    } else if (lig == 0) {
       double s = 0.0;
       for (int k = 0; k < K; k++) s = fma_(Q[k], R[k], s);
       f = fac * s;
@@ -150,30 +151,30 @@ struct Group {
       if (lig < n)
         for (int j = 0; j < n; j++) row[j] = 0.0;
       double jt = 0.0;
-      if (lig < N) {
-        const int e = sp_off[lig + 1];
-        for (int t = sp_off[lig]; t < e; t++) {
+      if (lig >= 1 && lig <= N) {
+        const int e = sp_off[sp + 1];
+        for (int t = sp_off[sp]; t < e; t++) {
           const int k = sp_k[t];
           const double dy = sp_dy[t];
           const int4 rpk = reinterpret_cast<const int4 *>(rp)[k];
           const int nslot = (rpk.x >> 8) & 0xff;
           const int c0 = rpk.z & 0xff, c1 = (rpk.z >> 8) & 0xff, c2 = (rpk.z >> 16) & 0xff;
-          row[c0] = fma_(dy, dRdY[3 * k], row[c0]);
-          if (nslot > 1) row[c1] = fma_(dy, dRdY[3 * k + 1], row[c1]);
-          if (nslot > 2) row[c2] = fma_(dy, dRdY[3 * k + 2], row[c2]);
-          row[N] = fma_(dy, dRdT[k], row[N]);
+          row[c0 + 1] = fma_(dy, dRdY[3 * k], row[c0 + 1]);
+          if (nslot > 1) row[c1 + 1] = fma_(dy, dRdY[3 * k + 1], row[c1 + 1]);
+          if (nslot > 2) row[c2 + 1] = fma_(dy, dRdY[3 * k + 2], row[c2 + 1]);
+          row[0] = fma_(dy, dRdT[k], row[0]);
         }
         // my column of the temperature row: sum_k Q_k dR_k/dY_lig, k ascending
-        const int ce = cl_off[lig + 1];
-        for (int c = cl_off[lig]; c < ce; c++) {
+        const int ce = cl_off[sp + 1];
+        for (int c = cl_off[sp]; c < ce; c++) {
           const int ks = cl_ks[c];
           jt = fma_(Q[ks & 0xffff], dRdY[3 * (ks & 0xffff) + (ks >> 16)], jt);
         }
-      } else if (lig == N) {
+      } else if (lig == 0) {
         for (int k = 0; k < K; k++) jt = fma_(Q[k], dRdT[k], jt);
       }
       sync();  // rows of the species are complete before the T row is written
-      if (lig < n) M[N * LD + lig] = fac * jt;
+      if (lig < n) M[lig] = fac * jt;  // row 0 = temperature equation
       sync();
     }
     return f;

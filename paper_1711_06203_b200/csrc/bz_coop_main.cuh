@@ -58,14 +58,14 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
     // ---- a1: load zone state -------------------------------------------------------------------
     const double rho = A.rho[z];
     double xin = 0.0, ai = 1.0;
-    if (lig < N) {
-      xin = A.X[(long long)lig * A.nz + z];
-      ai = g.aion[lig];
-    } else if (lig == N) {
+    if (lig >= 1 && lig <= N) {  // internal order: lane 0 = T, lane i + 1 = species i
+      xin = A.X[(long long)(lig - 1) * A.nz + z];
+      ai = g.aion[lig - 1];
+    } else if (lig == 0) {
       xin = A.T[z];
     }
-    const double y0 = (lig < N) ? xin / ai : xin;
-    bool bad = !(rho > 0.0) || !finite_(rho) || (act && !finite_(y0)) || (lig == N && !(y0 > 0.0));
+    const double y0 = (lig >= 1 && lig <= N) ? xin / ai : xin;
+    bool bad = !(rho > 0.0) || !finite_(rho) || (act && !finite_(y0)) || (lig == 0 && !(y0 > 0.0));
     int code = 0;
     double yfin = y0;
     if (g.gany(bad)) {
@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
           nord_predict(Z, q);  // B.2
           bool ok = false;
           double y = Z[0];
-          bool inval = (act && !finite_(y)) || (lig == N && !(y > 0.0));
+          bool inval = (act && !finite_(y)) || (lig == 0 && !(y > 0.0));
           if (!g.gany(inval)) {  // B.3
             f = g.template rates<true>(rho, y);
             c_rhs++, c_jac++;
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
               for (int m = 0; m < MAXCOR; m++) {
                 if (m > 0) {
                   y = Z[0] + acor;
-                  inval = (act && !finite_(y)) || (lig == N && !(y > 0.0));
+                  inval = (act && !finite_(y)) || (lig == 0 && !(y > 0.0));
                   if (g.gany(inval)) break;
                   f = g.template rates<false>(rho, y);
                   c_rhs++;
@@ -370,9 +370,9 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
     }
     // ---- a9: store ---------------------------------------------------------------------------
     if (code < 0) c_fail++;
-    if (lig < N) {
-      A.X_out[(long long)lig * A.nz + z] = (code == -4) ? xin : ai * yfin;
-    } else if (lig == N) {
+    if (lig >= 1 && lig <= N) {
+      A.X_out[(long long)(lig - 1) * A.nz + z] = (code == -4) ? xin : ai * yfin;
+    } else if (lig == 0) {
       A.T_out[z] = (code == -4) ? xin : yfin;
       A.nsteps[z] = code;
     }
