@@ -10,7 +10,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
 EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_host", "net_destroy", "bz_get_counters",
-                    "bz_norm_lanes", "bz_kernel_name", "bz_last_cuda_error", "bz_fp64_peak_probe")
+                    "bz_norm_lanes", "bz_select_kernel", "bz_kernel_name", "bz_last_cuda_error", "bz_fp64_peak_probe")
 _STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
            -5: "CUDA runtime error", -6: "out of memory"}
 
@@ -63,6 +63,8 @@ def _L():
         lib.bz_get_counters.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
         lib.bz_norm_lanes.restype = C.c_int
         lib.bz_norm_lanes.argtypes = [vp]
+        lib.bz_select_kernel.restype = C.c_int
+        lib.bz_select_kernel.argtypes = [vp, C.c_int]
         lib.bz_kernel_name.restype = C.c_char_p
         lib.bz_kernel_name.argtypes = [vp]
         lib.bz_last_cuda_error.restype = C.c_int
@@ -92,6 +94,10 @@ class Net:
     @property
     def kernel_name(self) -> str:
         return _L().bz_kernel_name(self._h).decode()
+
+    def select_kernel(self, kind: str = "auto") -> None:
+        """'auto' (specialised thread-per-zone kernel when available) or 'coop' (generic)."""
+        _check(_L().bz_select_kernel(self._h, {"auto": 0, "coop": 1}[kind]), "bz_select_kernel")
 
     def close(self):
         if self._h is not None:

@@ -12,6 +12,8 @@
 
 #include "../../include/burnzones.h"
 #include "bz_coop_main.cuh"
+#include "bz_tpz_main.cuh"
+#include "gen/registry.inc"
 
 namespace {
 
@@ -48,6 +50,50 @@ double host_log(double x) {
 }
 
 typedef void (*KernelFn)(bz::DevNet, bz::BurnArgs);
+typedef void (*TpzKernelFn)(bz::TpzNet, bz::BurnArgs, double *);
+
+// ---- network-specialised thread-per-zone kernels (generated topologies) -----------------------
+constexpr int TPZ_BLOCK = 32, TPZ_W = 4;
+struct TpzVariant {
+  const char *name;
+  unsigned long long topo_hash;
+  int neq, K, smem_bytes;
+  TpzKernelFn fn;
+};
+template <class Net>
+TpzVariant make_tpz(const char *name) {
+  const int tab = (4 * Net::K + Net::N + 1) & ~1;
+  return {name, Net::TOPO_HASH, Net::NEQ, Net::K,
+          (int)sizeof(double) * (tab + bz::TpzMem<Net::NEQ, TPZ_BLOCK>::PER_THREAD * TPZ_BLOCK),
+          (TpzKernelFn)bz::burn_tpz_kernel<Net, TPZ_BLOCK, TPZ_W>};
+}
+#define BZ_TPZ_ENTRY(NET) make_tpz<NET>("burn_tpz<" #NET ">"),
+const TpzVariant kTpz[] = {BZ_TPZ_NETS(BZ_TPZ_ENTRY)};
+
+// FNV-1a over the topology; must equal paper_1711_06203_b200/codegen.py:topology_hash
+unsigned long long topology_hash(const bz_net_desc *d) {
+  unsigned long long h = 0xcbf29ce484222325ull;
+  auto mix = [&](long long v) {
+    for (int b = 0; b < 8; b++) {
+      h ^= (unsigned long long)((v >> (8 * b)) & 0xff);
+      h *= 0x100000001b3ull;
+    }
+  };
+  mix(d->nspec);
+  mix(d->nreac);
+  for (int k = 0; k < d->nreac; k++) {
+    for (int a = 0; a < 3; a++) mix(d->reactant[3 * k + a]);
+    for (int a = 0; a < 4; a++) {
+      const int sid = d->stoich_id[4 * k + a];
+      mix(sid);
+      const double dy = sid >= 0 ? d->stoich_dy[4 * k + a] : 0.0;
+      long long bits;
+      std::memcpy(&bits, &dy, 8);
+      mix(bits);
+    }
+  }
+  return h;
+}
 
 struct Variant {
   const char *name;
@@ -83,6 +129,11 @@ struct bz_net {
   unsigned long long *d_scratch;  // [0] queue head, [1..8] counters
   const Variant *variant;
   int grid, smem_bytes;
+  const TpzVariant *tpz;  // non-null: a specialised kernel exists for this topology
+  int tpz_grid;
+  double *d_tpz_coef, *d_tpz_S;
+  double fac;
+  int force_coop;
   // staging for burn_zones_host
   double *st_in, *st_out;
   int32_t *st_nsteps;
@@ -216,6 +267,34 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     return fail(BZ_ERR_CUDA);
   if (bps < 1) return fail(BZ_ERR_NOMEM);
   h->grid = sms * bps;
+  h->fac = h->dev.fac;
+
+  // ---- specialised thread-per-zone kernel for known topologies ------------------------------------
+  const unsigned long long th = topology_hash(d);
+  for (const TpzVariant &v : kTpz)
+    if (v.topo_hash == th && v.neq == n && v.K == K) h->tpz = &v;
+  if (h->tpz) {
+    std::vector<double> tc;
+    tc.insert(tc.end(), lnA.begin(), lnA.end());
+    tc.insert(tc.end(), d->rate_n, d->rate_n + K);
+    tc.insert(tc.end(), d->rate_B, d->rate_B + K);
+    tc.insert(tc.end(), d->q_mev, d->q_mev + K);
+    tc.insert(tc.end(), d->aion, d->aion + N);
+    if (!cuda_ok(cudaMalloc(&h->d_tpz_coef, tc.size() * sizeof(double)))) return fail(BZ_ERR_CUDA);
+    if (!cuda_ok(cudaMemcpy(h->d_tpz_coef, tc.data(), tc.size() * sizeof(double), cudaMemcpyHostToDevice)))
+      return fail(BZ_ERR_CUDA);
+    int tb = 0;
+    if (!cuda_ok(cudaFuncSetAttribute((const void *)h->tpz->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      h->tpz->smem_bytes)))
+      return fail(BZ_ERR_CUDA);
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&tb, (const void *)h->tpz->fn, TPZ_BLOCK,
+                                                               h->tpz->smem_bytes)))
+      return fail(BZ_ERR_CUDA);
+    if (tb < 1) return fail(BZ_ERR_NOMEM);
+    h->tpz_grid = sms * tb;
+    if (!cuda_ok(cudaMalloc(&h->d_tpz_S, (size_t)n * h->tpz_grid * TPZ_BLOCK * sizeof(double))))
+      return fail(BZ_ERR_CUDA);
+  }
   *out = h;
   return BZ_OK;
 }
@@ -225,6 +304,8 @@ int net_destroy(bz_net *h) {
   if (h->d_dbl) cudaFree(h->d_dbl);
   if (h->d_int) cudaFree(h->d_int);
   if (h->d_scratch) cudaFree(h->d_scratch);
+  if (h->d_tpz_coef) cudaFree(h->d_tpz_coef);
+  if (h->d_tpz_S) cudaFree(h->d_tpz_S);
   if (h->st_in) cudaFree(h->st_in);
   if (h->st_out) cudaFree(h->st_out);
   if (h->st_nsteps) cudaFree(h->st_nsteps);
@@ -232,8 +313,15 @@ int net_destroy(bz_net *h) {
   return BZ_OK;
 }
 
-int bz_norm_lanes(const bz_net *h) { return h ? h->variant->lanes : BZ_ERR_NULL; }
-const char *bz_kernel_name(const bz_net *h) { return h ? h->variant->name : ""; }
+static bool use_tpz(const bz_net *h) { return h->tpz && !h->force_coop; }
+int bz_norm_lanes(const bz_net *h) { return h ? (use_tpz(h) ? 4 : h->variant->lanes) : BZ_ERR_NULL; }
+const char *bz_kernel_name(const bz_net *h) { return h ? (use_tpz(h) ? h->tpz->name : h->variant->name) : ""; }
+int bz_select_kernel(bz_net *h, int kind) {
+  if (!h) return BZ_ERR_NULL;
+  if (kind != 0 && kind != 1) return BZ_ERR_SIZE;
+  h->force_coop = kind;
+  return BZ_OK;
+}
 
 int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
                double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
@@ -251,6 +339,18 @@ int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, 
   a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
+  if (use_tpz(h)) {
+    bz::TpzNet tn;
+    tn.coef = h->d_tpz_coef;
+    tn.fac = h->fac;
+    const long long blocks_needed = (nz + TPZ_BLOCK - 1) / TPZ_BLOCK;
+    const int grid = (int)(blocks_needed < h->tpz_grid ? blocks_needed : h->tpz_grid);
+    double *S = h->d_tpz_S;
+    void *targs[] = {(void *)&tn, (void *)&a, (void *)&S};
+    BZ_CUDA(cudaLaunchKernel((const void *)h->tpz->fn, dim3(grid), dim3(TPZ_BLOCK), targs,
+                             (size_t)h->tpz->smem_bytes, st));
+    return BZ_OK;
+  }
   const int L = h->variant->lanes;
   const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
   const int grid = (int)(groups_needed < h->grid ? groups_needed : h->grid);

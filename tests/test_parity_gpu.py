@@ -17,10 +17,11 @@ pytestmark = pytest.mark.gpu
 OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
 
 
-def _gpu_burn(w, rho=None, T=None, X=None):
+def _gpu_burn(w, rho=None, T=None, X=None, kind="auto"):
     import torch
     import paper_1711_06203_b200 as bz
     net = bz.net_create(w.net)
+    net.select_kernel(kind)
     dev = torch.device("cuda:0")
     rho_d = torch.from_numpy(w.rho if rho is None else rho).to(dev)
     T_d = torch.from_numpy(w.T if T is None else T).to(dev)
@@ -41,14 +42,20 @@ def _record(tag, stats):
 
 
 # sizes: several tiles (blocks x groups) and a ragged tail; the oracle finishes in seconds
+@pytest.mark.parametrize("kind", ["auto", "coop"])
 @pytest.mark.parametrize("config,zones", [(1, None), (2, 61), (3, 509), (5, 4099)])
-def test_parity_sampled_configs(config, zones):
+def test_parity_sampled_configs(config, zones, kind):
+    """auto = network-specialised thread-per-zone kernel where one exists (configs 1-4), else the
+    generic cooperative kernel; coop = the generic kernel forced."""
+    if kind == "coop" and config == 5:
+        pytest.skip("config 5 has no specialised kernel: auto already ran the cooperative one")
     w = make_workload(config, zones=zones)
-    To, Xo, ns, cnt, lanes, name = _gpu_burn(w)
+    To, Xo, ns, cnt, lanes, name = _gpu_burn(w, kind=kind)
+    assert name.startswith("burn_coop") == (kind == "coop" or config == 5)
     Tr, Xr, nr, cr = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=lanes)
     stats = compare(To, Xo, ns, Tr, Xr, nr)
     stats.update(kernel=name, counters_equal=all(cnt[k] == cr[k] for k in cnt))
-    _record(f"config{config}", stats)
+    _record(f"config{config}:{kind}", stats)
     assert stats["nsteps_equal"] > 0.99
     # mass invariant on the GPU result itself (north_star: 1e-10)
     ok = ns > 0
