@@ -101,9 +101,11 @@ int bz_get_counters(const bz_net *net, void *cuda_stream, uint64_t out[8]);
  * Returns the lane count (>0) or a negative bz_status. */
 int bz_norm_lanes(const bz_net *net);
 
-/* Kernel selection: kind 0 = automatic (a network-specialised thread-per-zone kernel if the
+/* Kernel selection: kind 0 = automatic (the network-specialised 4-lanes-per-zone kernel if the
  * topology has one compiled in, else the generic cooperative kernel), 1 = always the generic
- * cooperative kernel.  Both follow the same arithmetic; only bz_norm_lanes differs. */
+ * cooperative kernel, 2 = the specialised thread-per-zone kernel, 3 = the specialised quad
+ * kernel (2 and 3 fall back to the cooperative kernel when the topology has none).  All follow
+ * the same arithmetic; only bz_norm_lanes differs. */
 int bz_select_kernel(bz_net *net, int kind);
 
 /* Name of the kernel variant burn_zones launches for this network (static string). */

@@ -96,8 +96,8 @@ class Net:
         return _L().bz_kernel_name(self._h).decode()
 
     def select_kernel(self, kind: str = "auto") -> None:
-        """'auto' (specialised thread-per-zone kernel when available) or 'coop' (generic)."""
-        _check(_L().bz_select_kernel(self._h, {"auto": 0, "coop": 1}[kind]), "bz_select_kernel")
+        """'auto' (specialised quad kernel when available), 'coop' (generic), 'tpz', 'quad'."""
+        _check(_L().bz_select_kernel(self._h, {"auto": 0, "coop": 1, "tpz": 2, "quad": 3}[kind]), "bz_select_kernel")
 
     def close(self):
         if self._h is not None:

@@ -1,0 +1,184 @@
+// bz_quad.cuh -- 4 lanes per zone ("quad") burn kernel pieces, DESIGN.md section 5.3.
+//
+// Why 4 lanes: a zone's integrator state is ~3 KB (n = 14: P/LU 196, Z 84, vectors ~60 doubles),
+// so only ~100-130 zones fit on an SM.  One thread per zone then means 3-4 warps per SM and every
+// instruction latency is exposed (measured: 1.6 % of FP64 peak).  Splitting a zone over 4 lanes
+// gives 12-16 resident warps with the same state, 4 independent slots of work per lane, and short
+// dependent chains -- at the price of a few shuffles and some redundant scalar arithmetic.
+//
+// Mapping: component i of every n-vector lives on lane c = i % 4 of the quad, slot s = i / 4;
+// ROW i of the Newton matrix P lives in the same place (a[s][0..n-1], registers, static indices).
+// The Nordsieck array, weights and the saved vector live in shared memory per zone.
+// LU (a5): the unknowns are ordered temperature-first, so partial pivoting
+// keeps the natural order almost always: step k's pivot row is the static (lane k%4, slot k/4);
+// it is published through shared memory, every lane verifies |a_ik| <= |a_kk| on its own rows
+// (exact), computes its own multipliers and updates its own rows.  A zone that does need an
+// interchange redoes the factorisation on the general path (lane 0 of the quad, LINPACK dgefa on
+// a global-memory scratch copy), bit-identical to the oracle either way.
+#pragma once
+#include <cstdint>
+#include "bz_coop.cuh"      // constants, BurnArgs, eta_of, factorial_, inv_small_int
+#include "bz_coop_burn.cuh" // nord_predict / nord_retract / nord_rescale / build_d / sel
+
+namespace bz {
+
+struct QuadNet {
+  const double *coef;  // device: lnA[K] n[K] B[K] Q[K] aion[N]
+  double fac;
+  double *gscratch;    // device: per-quad general-path scratch, NEQ*NEQ + NEQ doubles + NEQ ints each
+};
+
+// per-zone shared memory (doubles); size padded so that consecutive zones start 4 doubles apart
+// modulo 32 (8 zones x 4 lanes x 8 B of a warp access then cover all banks exactly twice)
+template <int NEQ, int K>
+struct QuadMem {
+  static constexpr int Z_OFF = 0;                       // Z[6][NEQ]
+  static constexpr int W_OFF = Z_OFF + (QMAX + 1) * NEQ; // w[NEQ]
+  static constexpr int S_OFF = W_OFF + NEQ;             // saved vector S[NEQ]
+  static constexpr int Y_OFF = S_OFF + NEQ;             // y / f gather [NEQ]
+  static constexpr int U_OFF = Y_OFF + NEQ;             // pivot row broadcast, 2 x NEQ
+  static constexpr int L_OFF = U_OFF + 2 * NEQ;         // lambda_k [K]
+  static constexpr int RAW = L_OFF + K;
+  static constexpr int SIZE = RAW + ((4 - (RAW % 32) + 32) % 32);  // == 4 (mod 32)
+  double *base;
+  __device__ __forceinline__ double &Z(int j, int i) const { return base[Z_OFF + j * NEQ + i]; }
+  __device__ __forceinline__ double &W(int i) const { return base[W_OFF + i]; }
+  __device__ __forceinline__ double &Sv(int i) const { return base[S_OFF + i]; }
+  __device__ __forceinline__ double *ysh() const { return base + Y_OFF; }
+  __device__ __forceinline__ double *ub(int par) const { return base + U_OFF + par * NEQ; }
+  __device__ __forceinline__ double *lam() const { return base + L_OFF; }
+};
+
+template <int NEQ>
+struct QuadLU {
+  static constexpr int S = (NEQ + 3) / 4;
+  double a[S][NEQ];  // my rows of P, then of its LU factors (l_ik below the diagonal, U above)
+  double invd[S];    // 1/pivot of my rows
+
+  __device__ __forceinline__ static unsigned hi_abs(double x) {
+    return (unsigned)(__double_as_longlong(x) >> 32) & 0x7fffffffu;
+  }
+
+  // no-interchange factorisation.  returns bit 0: an interchange was needed (results invalid),
+  // bit 1: zero / NaN pivot.  Quad-uniform result.
+  template <class Mem>
+  __device__ __forceinline__ unsigned factor(const Mem &m, int c, unsigned gmask) {
+    bool swap_needed = false, bad = false;
+#pragma unroll
+    for (int k = 0; k < NEQ; k++) {
+      constexpr int dummy = 0;
+      (void)dummy;
+      const int ko = k & 3, ks = k >> 2;
+      double *ub = m.ub(k & 1);
+      if (c == ko) {
+#pragma unroll
+        for (int j = k; j < NEQ; j++) ub[j] = a[ks][j];
+      }
+      __syncwarp(gmask);
+      const double piv = ub[k];
+      const unsigned hk = hi_abs(piv);
+      bad |= !(fabs(piv) > 0.0);
+      const double inv = 1.0 / piv;
+      if (c == ko) invd[ks] = inv;
+#pragma unroll
+      for (int s = 0; s < S; s++) {
+        if (s < ks) continue;
+        const bool mine = (s > ks) || (c > ko);  // row 4s+c is below the pivot row
+        if (mine) {
+          const double v = a[s][k];
+          if (hi_abs(v) >= hk) swap_needed |= (fabs(v) > fabs(piv));
+          const double l = v * inv;
+          a[s][k] = l;
+#pragma unroll
+          for (int j = k + 1; j < NEQ; j++) a[s][j] = fma_(-l, ub[j], a[s][j]);
+        }
+      }
+    }
+    const unsigned f = (swap_needed ? 1u : 0u) | (bad ? 2u : 0u);
+    // make the flags quad-uniform
+    unsigned r = f;
+    r |= __shfl_xor_sync(gmask, r, 1, 4);
+    r |= __shfl_xor_sync(gmask, r, 2, 4);
+    return r;
+  }
+
+  // dgesl without interchanges: b[s] = my components of the right-hand side / solution
+  __device__ __forceinline__ void solve(int c, unsigned gmask, double (&b)[S]) const {
+#pragma unroll
+    for (int k = 0; k < NEQ; k++) {
+      const int ko = k & 3, ks = k >> 2;
+      const double bk = __shfl_sync(gmask, b[ks], ko, 4);
+#pragma unroll
+      for (int s = 0; s < S; s++) {
+        if (s < ks) continue;
+        if ((s > ks) || (c > ko)) b[s] = fma_(-a[s][k], bk, b[s]);
+      }
+    }
+#pragma unroll
+    for (int k = NEQ - 1; k >= 0; k--) {
+      const int ko = k & 3, ks = k >> 2;
+      const double x = b[ks] * invd[ks];
+      if (c == ko) b[ks] = x;
+      const double xk = __shfl_sync(gmask, x, ko, 4);
+#pragma unroll
+      for (int s = 0; s < S; s++) {
+        if (s > ks) continue;
+        if ((s < ks) || (c < ko)) b[s] = fma_(-a[s][k], xk, b[s]);
+      }
+    }
+  }
+};
+
+// ---- general path (rare): LINPACK dgefa / dgesl on a row-major n x n matrix in global memory ----
+template <int NEQ>
+__device__ __noinline__ bool quad_lu_general(double *P, int *ipvt) {
+  bool ok = true;
+  for (int k = 0; k < NEQ; k++) {
+    int p = k;
+    double amax = fabs(P[k * NEQ + k]);
+    for (int i = k + 1; i < NEQ; i++) {
+      const double v = fabs(P[i * NEQ + k]);
+      if (v > amax) {
+        amax = v;
+        p = i;
+      }
+    }
+    ipvt[k] = p;
+    if (!(amax > 0.0)) {
+      ok = false;
+      P[k * NEQ + k] = 0.0;
+      continue;
+    }
+    if (p != k)
+      for (int j = k; j < NEQ; j++) {
+        const double t = P[p * NEQ + j];
+        P[p * NEQ + j] = P[k * NEQ + j];
+        P[k * NEQ + j] = t;
+      }
+    const double inv = 1.0 / P[k * NEQ + k];
+    for (int i = k + 1; i < NEQ; i++) P[i * NEQ + k] = P[i * NEQ + k] * inv;
+    for (int i = k + 1; i < NEQ; i++) {
+      const double l = P[i * NEQ + k];
+      for (int j = k + 1; j < NEQ; j++) P[i * NEQ + j] = fma_(-l, P[k * NEQ + j], P[i * NEQ + j]);
+    }
+    P[k * NEQ + k] = inv;  // 1/pivot on the diagonal
+  }
+  return ok;
+}
+template <int NEQ>
+__device__ __noinline__ void quad_solve_general(const double *P, const int *ipvt, double *b) {
+  for (int k = 0; k < NEQ; k++) {
+    const int p = ipvt[k];
+    const double t = b[p];
+    b[p] = b[k];
+    b[k] = t;
+    for (int i = k + 1; i < NEQ; i++) b[i] = fma_(-P[i * NEQ + k], t, b[i]);
+  }
+  for (int k = NEQ - 1; k >= 0; k--) {
+    b[k] = b[k] * P[k * NEQ + k];
+    const double t = b[k];
+    for (int i = 0; i < k; i++) b[i] = fma_(-P[i * NEQ + k], t, b[i]);
+  }
+}
+
+}  // namespace bz

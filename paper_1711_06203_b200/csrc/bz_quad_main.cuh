@@ -1,0 +1,160 @@
+// bz_quad_main.cuh -- quad kernel entry: work queue + BZ-BDF v1 driver, one loop trip = one
+// step attempt of the quad's zone (flat state machine, see bz_quad.cuh for the mapping).
+#pragma once
+#include "bz_quad.cuh"
+
+namespace bz {
+
+constexpr int QUAD_THREADS = 128;
+
+template <class Net, int MINB>
+__global__ void __launch_bounds__(QUAD_THREADS, MINB) burn_quad_kernel(QuadNet qn, BurnArgs A) {
+  constexpr int NEQ = Net::NEQ, N = Net::N, K = Net::K, S = Net::S;
+  typedef QuadMem<NEQ, K> Mem;
+  extern __shared__ __align__(16) double smem[];
+  double *coef = smem;  // lnA n B Q [4K] + aion [N]
+  for (int i = threadIdx.x; i < 4 * K + N; i += QUAD_THREADS) coef[i] = qn.coef[i];
+  __syncthreads();
+  const double *aion = coef + 4 * K;
+  const int c = threadIdx.x & 3;
+  const unsigned gmask = 0xfu << ((threadIdx.x & 31) & ~3);
+  Mem m;
+  m.base = smem + ((4 * K + N + 1) & ~1) + (threadIdx.x >> 2) * Mem::SIZE;
+  const long long gquad = (long long)blockIdx.x * (QUAD_THREADS / 4) + (threadIdx.x >> 2);
+  double *gP = qn.gscratch + gquad * (NEQ * NEQ + 2 * NEQ);  // general path: P, b, ipvt
+  const double dt = A.dt, rtol = A.rtol, atol = A.atol, fac = qn.fac;
+  const double inv_n = 1.0 / (double)NEQ;
+  unsigned long long c_nst = 0, c_rhs = 0, c_jac = 0, c_lu = 0, c_sol = 0, c_etf = 0, c_cfn = 0, c_fail = 0;
+
+  // component index of my slot s and its validity
+#define BZQ_I(s) (4 * (s) + c)
+#define BZQ_OK(s) (4 * (s) + c < NEQ)
+
+  auto qsum = [&](double v) {  // quad butterfly, strides 2 then 1 (norm_lanes = 4)
+    v = v + __shfl_xor_sync(gmask, v, 2, 4);
+    v = v + __shfl_xor_sync(gmask, v, 1, 4);
+    return v;
+  };
+  auto wrms = [&](const double (&v)[S]) {
+    double p = 0.0;
+#pragma unroll
+    for (int s = 0; s < S; s++)
+      if (BZQ_OK(s)) {
+        const double d = v[s] * m.W(BZQ_I(s));
+        p = fma_(d, d, p);
+      }
+    return sqrt(qsum(p) * inv_n);
+  };
+  auto qany = [&](bool p) { return (__ballot_sync(gmask, p) & gmask) != 0u; };
+
+  int phase = 0;  // 0 need a zone, 1 stepping, 2 queue empty
+  long long z = 0;
+  double rho = 0.0, h = 0.0, t = 0.0, etamax = ETAMX1, hS = 0.0;
+  int q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0, ncf = 0, nef = 0;
+  bool newstep = true, last = false;
+  double tau[QMAX + 1];
+#pragma unroll
+  for (int i = 0; i <= QMAX; i++) tau[i] = 0.0;
+  QuadLU<NEQ> lu;
+#pragma unroll
+  for (int s = 0; s < S; s++) lu.invd[s] = 0.0;
+
+  for (;;) {
+    if (phase == 0) {
+      // ---- a2 + a1: next zone, load, validate, initialise ------------------------------------------
+      if (c == 0) z = (long long)atomicAdd(A.queue, 1ull);
+      z = __shfl_sync(gmask, z, 0, 4);
+      if (z >= A.nz) {
+        phase = 2;
+      } else {
+        rho = A.rho[z];
+        double xin[S], y[S];
+        bool bad = !(rho > 0.0) || !finite_(rho);
+#pragma unroll
+        for (int s = 0; s < S; s++) {
+          const int i = BZQ_I(s);
+          xin[s] = 0.0;
+          y[s] = 0.0;
+          if (i == 0) {
+            xin[s] = A.T[z];
+            y[s] = xin[s];
+            bad |= !(y[s] > 0.0) || !finite_(y[s]);
+          } else if (i < NEQ) {
+            xin[s] = A.X[(long long)(i - 1) * A.nz + z];
+            y[s] = xin[s] / aion[i - 1];
+            bad |= !finite_(y[s]);
+          }
+        }
+        if (qany(bad)) {  // invalid input zone: outputs = inputs, stay in phase 0
+#pragma unroll
+          for (int s = 0; s < S; s++) {
+            const int i = BZQ_I(s);
+            if (i == 0) {
+              A.T_out[z] = xin[s];
+              A.nsteps[z] = -4;
+            } else if (i < NEQ)
+              A.X_out[(long long)(i - 1) * A.nz + z] = xin[s];
+          }
+          c_fail++;
+        } else {
+          double f[S], v[S];
+          __syncwarp(gmask);
+#pragma unroll
+          for (int s = 0; s < S; s++)
+            if (BZQ_OK(s)) {
+              m.ysh()[BZQ_I(s)] = y[s];
+              m.W(BZQ_I(s)) = 1.0 / fma_(rtol, fabs(y[s]), atol);
+              m.Z(0, BZQ_I(s)) = y[s];
+            }
+          __syncwarp(gmask);
+          Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, f, lu.a);
+          c_rhs++, c_jac++;
+          // exact second derivative y'' = J f for the first step size
+          __syncwarp(gmask);
+#pragma unroll
+          for (int s = 0; s < S; s++)
+            if (BZQ_OK(s)) m.ysh()[BZQ_I(s)] = f[s];
+          __syncwarp(gmask);
+#pragma unroll
+          for (int s = 0; s < S; s++) {
+            double acc = 0.0;
+#pragma unroll
+            for (int j = 0; j < NEQ; j++) acc = fma_(lu.a[s][j], m.ysh()[j], acc);
+            v[s] = acc;
+          }
+          const double d2 = wrms(v);
+          h = dt;
+          if (d2 > 0.0) {
+            const double hh = 0.5 * sqrt(2.0 / d2);
+            if (hh < dt) h = hh;
+          }
+#pragma unroll
+          for (int s = 0; s < S; s++)
+            if (BZQ_OK(s)) m.Z(1, BZQ_I(s)) = h * f[s];
+          q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0;
+          t = 0.0, etamax = ETAMX1, hS = 0.0;
+#pragma unroll
+          for (int i = 0; i <= QMAX; i++) tau[i] = 0.0;
+          newstep = true;
+          phase = 1;
+        }
+      }
+    }
+    if (__all_sync(0xffffffffu, phase == 2)) break;
+    if (phase != 1) continue;
+#include "bz_quad_attempt.inc"
+  }
+#undef BZQ_I
+#undef BZQ_OK
+  // ---- counters (lane 0 of each quad holds the zone's counts) ------------------------------------
+  unsigned long long cs[8] = {c_nst, c_rhs, c_jac, c_lu, c_sol, c_etf, c_cfn, c_fail};
+#pragma unroll
+  for (int k = 0; k < 8; k++) {
+    unsigned long long v = (c == 0) ? cs[k] : 0ull;
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+    if ((threadIdx.x & 31) == 0) atomicAdd(A.counters + k, v);
+  }
+}
+
+}  // namespace bz

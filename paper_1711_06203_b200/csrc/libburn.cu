@@ -13,6 +13,7 @@
 #include "../../include/burnzones.h"
 #include "bz_coop_main.cuh"
 #include "bz_tpz_main.cuh"
+#include "bz_quad_main.cuh"
 #include "gen/registry.inc"
 
 namespace {
@@ -67,6 +68,28 @@ TpzVariant make_tpz(const char *name) {
           (int)sizeof(double) * (tab + bz::TpzMem<Net::NEQ, TPZ_BLOCK>::PER_THREAD * TPZ_BLOCK),
           (TpzKernelFn)bz::burn_tpz_kernel<Net, TPZ_BLOCK, TPZ_W>};
 }
+typedef void (*QuadKernelFn)(bz::QuadNet, bz::BurnArgs);
+struct QuadVariant {
+  const char *name;
+  unsigned long long topo_hash;
+  int neq, K, smem_bytes;
+  QuadKernelFn fn;
+};
+template <class Net, int MINB>
+QuadVariant make_quad(const char *name) {
+  const int tab = (4 * Net::K + Net::N + 1) & ~1;
+  return {name, Net::TOPO_HASH, Net::NEQ, Net::K,
+          (int)sizeof(double) * (tab + bz::QuadMem<Net::NEQ, Net::K>::SIZE * (bz::QUAD_THREADS / 4)),
+          (QuadKernelFn)bz::burn_quad_kernel<Net, MINB>};
+}
+// two register budgets: 3 blocks/SM (<= 168 registers) and 2 blocks/SM (<= 255 registers);
+// BZ_QUAD_MINB=2|3 in the environment picks one at net_create (tuning knob, default below)
+#define BZ_QUAD_ENTRY3(NET) make_quad<NET, 3>("burn_quad<" #NET ",3>"),
+#define BZ_QUAD_ENTRY2(NET) make_quad<NET, 2>("burn_quad<" #NET ",2>"),
+const QuadVariant kQuad3[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY3)};
+const QuadVariant kQuad2[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY2)};
+constexpr int QUAD_MINB_DEFAULT = 3;
+
 #define BZ_TPZ_ENTRY(NET) make_tpz<NET>("burn_tpz<" #NET ">"),
 const TpzVariant kTpz[] = {BZ_TPZ_NETS(BZ_TPZ_ENTRY)};
 
@@ -132,8 +155,11 @@ struct bz_net {
   const TpzVariant *tpz;  // non-null: a specialised kernel exists for this topology
   int tpz_grid;
   double *d_tpz_coef, *d_tpz_S;
+  const QuadVariant *quad;
+  int quad_grid;
+  double *d_quad_scratch;
   double fac;
-  int force_coop;
+  int kind;  // 0 auto, 1 cooperative, 2 thread-per-zone, 3 quad
   // staging for burn_zones_host
   double *st_in, *st_out;
   int32_t *st_nsteps;
@@ -294,6 +320,26 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     h->tpz_grid = sms * tb;
     if (!cuda_ok(cudaMalloc(&h->d_tpz_S, (size_t)n * h->tpz_grid * TPZ_BLOCK * sizeof(double))))
       return fail(BZ_ERR_CUDA);
+    int minb = QUAD_MINB_DEFAULT;
+    if (const char *e = std::getenv("BZ_QUAD_MINB")) minb = std::atoi(e);
+    const QuadVariant *tab = (minb == 2) ? kQuad2 : kQuad3;
+    const int ntab = (int)(sizeof(kQuad3) / sizeof(kQuad3[0]));
+    for (int i = 0; i < ntab; i++)
+      if (tab[i].topo_hash == th && tab[i].neq == n && tab[i].K == K) h->quad = &tab[i];
+  }
+  if (h->quad) {
+    int qb = 0;
+    if (!cuda_ok(cudaFuncSetAttribute((const void *)h->quad->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      h->quad->smem_bytes)))
+      return fail(BZ_ERR_CUDA);
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&qb, (const void *)h->quad->fn, bz::QUAD_THREADS,
+                                                               h->quad->smem_bytes)))
+      return fail(BZ_ERR_CUDA);
+    if (qb < 1) return fail(BZ_ERR_NOMEM);
+    h->quad_grid = sms * qb;
+    const size_t per_quad = (size_t)n * n + 2 * n;
+    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * h->quad_grid * (bz::QUAD_THREADS / 4) * sizeof(double))))
+      return fail(BZ_ERR_CUDA);
   }
   *out = h;
   return BZ_OK;
@@ -306,6 +352,7 @@ int net_destroy(bz_net *h) {
   if (h->d_scratch) cudaFree(h->d_scratch);
   if (h->d_tpz_coef) cudaFree(h->d_tpz_coef);
   if (h->d_tpz_S) cudaFree(h->d_tpz_S);
+  if (h->d_quad_scratch) cudaFree(h->d_quad_scratch);
   if (h->st_in) cudaFree(h->st_in);
   if (h->st_out) cudaFree(h->st_out);
   if (h->st_nsteps) cudaFree(h->st_nsteps);
@@ -313,13 +360,18 @@ int net_destroy(bz_net *h) {
   return BZ_OK;
 }
 
-static bool use_tpz(const bz_net *h) { return h->tpz && !h->force_coop; }
-int bz_norm_lanes(const bz_net *h) { return h ? (use_tpz(h) ? 4 : h->variant->lanes) : BZ_ERR_NULL; }
-const char *bz_kernel_name(const bz_net *h) { return h ? (use_tpz(h) ? h->tpz->name : h->variant->name) : ""; }
+static bool use_quad(const bz_net *h) { return h->quad && (h->kind == 0 || h->kind == 3); }
+static bool use_tpz(const bz_net *h) { return h->tpz && h->kind == 2; }
+int bz_norm_lanes(const bz_net *h) {
+  return h ? ((use_quad(h) || use_tpz(h)) ? 4 : h->variant->lanes) : BZ_ERR_NULL;
+}
+const char *bz_kernel_name(const bz_net *h) {
+  return h ? (use_quad(h) ? h->quad->name : (use_tpz(h) ? h->tpz->name : h->variant->name)) : "";
+}
 int bz_select_kernel(bz_net *h, int kind) {
   if (!h) return BZ_ERR_NULL;
-  if (kind != 0 && kind != 1) return BZ_ERR_SIZE;
-  h->force_coop = kind;
+  if (kind < 0 || kind > 3) return BZ_ERR_SIZE;
+  h->kind = kind;
   return BZ_OK;
 }
 
@@ -339,6 +391,19 @@ int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, 
   a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
+  if (use_quad(h)) {
+    bz::QuadNet qn;
+    qn.coef = h->d_tpz_coef;
+    qn.fac = h->fac;
+    qn.gscratch = h->d_quad_scratch;
+    const int zpb = bz::QUAD_THREADS / 4;
+    const long long blocks_needed = (nz + zpb - 1) / zpb;
+    const int grid = (int)(blocks_needed < h->quad_grid ? blocks_needed : h->quad_grid);
+    void *qargs[] = {(void *)&qn, (void *)&a};
+    BZ_CUDA(cudaLaunchKernel((const void *)h->quad->fn, dim3(grid), dim3(bz::QUAD_THREADS), qargs,
+                             (size_t)h->quad->smem_bytes, st));
+    return BZ_OK;
+  }
   if (use_tpz(h)) {
     bz::TpzNet tn;
     tn.coef = h->d_tpz_coef;

@@ -42,16 +42,17 @@ def _record(tag, stats):
 
 
 # sizes: several tiles (blocks x groups) and a ragged tail; the oracle finishes in seconds
-@pytest.mark.parametrize("kind", ["auto", "coop"])
+@pytest.mark.parametrize("kind", ["auto", "coop", "tpz"])
 @pytest.mark.parametrize("config,zones", [(1, None), (2, 61), (3, 509), (5, 4099)])
 def test_parity_sampled_configs(config, zones, kind):
-    """auto = network-specialised thread-per-zone kernel where one exists (configs 1-4), else the
-    generic cooperative kernel; coop = the generic kernel forced."""
-    if kind == "coop" and config == 5:
+    """auto = network-specialised quad kernel where one exists (configs 1-4), else the generic
+    cooperative kernel; coop / tpz = the generic / thread-per-zone kernel forced."""
+    if kind != "auto" and config == 5:
         pytest.skip("config 5 has no specialised kernel: auto already ran the cooperative one")
     w = make_workload(config, zones=zones)
     To, Xo, ns, cnt, lanes, name = _gpu_burn(w, kind=kind)
-    assert name.startswith("burn_coop") == (kind == "coop" or config == 5)
+    want = "burn_coop" if (kind == "coop" or config == 5) else ("burn_tpz" if kind == "tpz" else "burn_quad")
+    assert name.startswith(want), name
     Tr, Xr, nr, cr = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=lanes)
     stats = compare(To, Xo, ns, Tr, Xr, nr)
     stats.update(kernel=name, counters_equal=all(cnt[k] == cr[k] for k in cnt))
