@@ -5,10 +5,13 @@
 
 namespace bz {
 
-constexpr int QUAD_THREADS = 128;
-
-template <class Net, int MINB>
-__global__ void __launch_bounds__(QUAD_THREADS, MINB) burn_quad_kernel(QuadNet qn, BurnArgs A) {
+// BLOCK threads = BLOCK/4 zones per block; MINB blocks per SM (register budget 65536/(BLOCK*MINB)).
+// All warps of a block meet at ONE barrier per loop trip (= per step attempt): that keeps them in
+// the same part of the ~100 KB loop body, so instruction-cache lines fetched by one warp are reused
+// by the others (unsynchronised warps thrashed the instruction cache: profiles/README.md).
+template <class Net, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, BurnArgs A) {
+  constexpr int QUAD_THREADS = BLOCK;
   constexpr int NEQ = Net::NEQ, N = Net::N, K = Net::K, S = Net::S;
   typedef QuadMem<NEQ, K> Mem;
   extern __shared__ __align__(16) double smem[];
@@ -29,6 +32,13 @@ __global__ void __launch_bounds__(QUAD_THREADS, MINB) burn_quad_kernel(QuadNet q
   // component index of my slot s and its validity
 #define BZQ_I(s) (4 * (s) + c)
 #define BZQ_OK(s) (4 * (s) + c < NEQ)
+  // optional barriers between the segments of an attempt (measured slower than one barrier per
+  // trip: they serialise the pipes; kept as a switch)
+#ifdef BZ_QUAD_SEGMENT_BARRIERS
+#define BZQ_SEG_SYNC() __syncthreads()
+#else
+#define BZQ_SEG_SYNC() ((void)0)
+#endif
 
   auto qsum = [&](double v) {  // quad butterfly, strides 2 then 1 (norm_lanes = 4)
     v = v + __shfl_xor_sync(gmask, v, 2, 4);
@@ -140,12 +150,12 @@ __global__ void __launch_bounds__(QUAD_THREADS, MINB) burn_quad_kernel(QuadNet q
         }
       }
     }
-    if (__all_sync(0xffffffffu, phase == 2)) break;
-    if (phase != 1) continue;
+    if (__syncthreads_and(phase == 2)) break;
 #include "bz_quad_attempt.inc"
   }
 #undef BZQ_I
 #undef BZQ_OK
+#undef BZQ_SEG_SYNC
   // ---- counters (lane 0 of each quad holds the zone's counts) ------------------------------------
   unsigned long long cs[8] = {c_nst, c_rhs, c_jac, c_lu, c_sol, c_etf, c_cfn, c_fail};
 #pragma unroll

@@ -82,7 +82,9 @@ __global__ void __launch_bounds__(BLOCK) burn_tpz_kernel(TpzNet tn, BurnArgs A, 
         }
       }
     }
-    if (__all_sync(0xffffffffu, phase == 2)) break;
+    // one block barrier per trip keeps the block's warps in the same part of the (large) loop body,
+    // so they share instruction-cache lines (profiles/README.md)
+    if (__syncthreads_and(phase == 2)) break;
     if (phase != 1) continue;
 
     // ================= one step attempt (C.2-A/B) =============================================

@@ -54,7 +54,7 @@ typedef void (*KernelFn)(bz::DevNet, bz::BurnArgs);
 typedef void (*TpzKernelFn)(bz::TpzNet, bz::BurnArgs, double *);
 
 // ---- network-specialised thread-per-zone kernels (generated topologies) -----------------------
-constexpr int TPZ_BLOCK = 32, TPZ_W = 4;
+constexpr int TPZ_BLOCK = 96, TPZ_W = 4;
 struct TpzVariant {
   const char *name;
   unsigned long long topo_hash;
@@ -72,23 +72,23 @@ typedef void (*QuadKernelFn)(bz::QuadNet, bz::BurnArgs);
 struct QuadVariant {
   const char *name;
   unsigned long long topo_hash;
-  int neq, K, smem_bytes;
+  int neq, K, smem_bytes, block;
   QuadKernelFn fn;
 };
-template <class Net, int MINB>
+template <class Net, int BLOCK, int MINB>
 QuadVariant make_quad(const char *name) {
   const int tab = (4 * Net::K + Net::N + 1) & ~1;
   return {name, Net::TOPO_HASH, Net::NEQ, Net::K,
-          (int)sizeof(double) * (tab + bz::QuadMem<Net::NEQ, Net::K>::SIZE * (bz::QUAD_THREADS / 4)),
-          (QuadKernelFn)bz::burn_quad_kernel<Net, MINB>};
+          (int)sizeof(double) * (tab + bz::QuadMem<Net::NEQ, Net::K>::SIZE * (BLOCK / 4)), BLOCK,
+          (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB>};
 }
-// two register budgets: 3 blocks/SM (<= 168 registers) and 2 blocks/SM (<= 255 registers);
-// BZ_QUAD_MINB=2|3 in the environment picks one at net_create (tuning knob, default below)
-#define BZ_QUAD_ENTRY3(NET) make_quad<NET, 3>("burn_quad<" #NET ",3>"),
-#define BZ_QUAD_ENTRY2(NET) make_quad<NET, 2>("burn_quad<" #NET ",2>"),
+// two block shapes with the same register budget (<= 168): 3 blocks of 128 threads per SM, or one
+// block of 384 threads per SM (all 12 warps share one barrier per trip = one instruction stream;
+// measured 1.8x faster, profiles/README.md).  BZ_QUAD_SHAPE=128x3|384x1 picks one at net_create.
+#define BZ_QUAD_ENTRY3(NET) make_quad<NET, 128, 3>("burn_quad<" #NET ",128x3>"),
+#define BZ_QUAD_ENTRY2(NET) make_quad<NET, 384, 1>("burn_quad<" #NET ",384x1>"),
 const QuadVariant kQuad3[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY3)};
 const QuadVariant kQuad2[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY2)};
-constexpr int QUAD_MINB_DEFAULT = 3;
 
 #define BZ_TPZ_ENTRY(NET) make_tpz<NET>("burn_tpz<" #NET ">"),
 const TpzVariant kTpz[] = {BZ_TPZ_NETS(BZ_TPZ_ENTRY)};
@@ -320,9 +320,9 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     h->tpz_grid = sms * tb;
     if (!cuda_ok(cudaMalloc(&h->d_tpz_S, (size_t)n * h->tpz_grid * TPZ_BLOCK * sizeof(double))))
       return fail(BZ_ERR_CUDA);
-    int minb = QUAD_MINB_DEFAULT;
-    if (const char *e = std::getenv("BZ_QUAD_MINB")) minb = std::atoi(e);
-    const QuadVariant *tab = (minb == 2) ? kQuad2 : kQuad3;
+    bool big = true;  // default: 384x1
+    if (const char *e = std::getenv("BZ_QUAD_SHAPE")) big = (std::strcmp(e, "128x3") != 0);
+    const QuadVariant *tab = big ? kQuad2 : kQuad3;
     const int ntab = (int)(sizeof(kQuad3) / sizeof(kQuad3[0]));
     for (int i = 0; i < ntab; i++)
       if (tab[i].topo_hash == th && tab[i].neq == n && tab[i].K == K) h->quad = &tab[i];
@@ -332,13 +332,13 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     if (!cuda_ok(cudaFuncSetAttribute((const void *)h->quad->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       h->quad->smem_bytes)))
       return fail(BZ_ERR_CUDA);
-    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&qb, (const void *)h->quad->fn, bz::QUAD_THREADS,
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&qb, (const void *)h->quad->fn, h->quad->block,
                                                                h->quad->smem_bytes)))
       return fail(BZ_ERR_CUDA);
     if (qb < 1) return fail(BZ_ERR_NOMEM);
     h->quad_grid = sms * qb;
     const size_t per_quad = (size_t)n * n + 2 * n;
-    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * h->quad_grid * (bz::QUAD_THREADS / 4) * sizeof(double))))
+    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * h->quad_grid * (h->quad->block / 4) * sizeof(double))))
       return fail(BZ_ERR_CUDA);
   }
   *out = h;
@@ -396,11 +396,11 @@ int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, 
     qn.coef = h->d_tpz_coef;
     qn.fac = h->fac;
     qn.gscratch = h->d_quad_scratch;
-    const int zpb = bz::QUAD_THREADS / 4;
+    const int zpb = h->quad->block / 4;
     const long long blocks_needed = (nz + zpb - 1) / zpb;
     const int grid = (int)(blocks_needed < h->quad_grid ? blocks_needed : h->quad_grid);
     void *qargs[] = {(void *)&qn, (void *)&a};
-    BZ_CUDA(cudaLaunchKernel((const void *)h->quad->fn, dim3(grid), dim3(bz::QUAD_THREADS), qargs,
+    BZ_CUDA(cudaLaunchKernel((const void *)h->quad->fn, dim3(grid), dim3(h->quad->block), qargs,
                              (size_t)h->quad->smem_bytes, st));
     return BZ_OK;
   }
