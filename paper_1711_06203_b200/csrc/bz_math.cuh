@@ -7,6 +7,14 @@
 
 namespace bz {
 
+// Polynomial coefficients live in constant memory so that each Horner step is ONE DFMA with a
+// constant-bank operand (as 64-bit immediates they cost two extra UMOV per step).
+__constant__ double EXP_C[14] = {1.0, 1.0, 1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0,
+                                 1.0 / 5040.0, 1.0 / 40320.0, 1.0 / 362880.0, 1.0 / 3628800.0,
+                                 1.0 / 39916800.0, 1.0 / 479001600.0, 1.0 / 6227020800.0};
+__constant__ double LOG_C[12] = {1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0,
+                                 1.0 / 15.0, 1.0 / 17.0, 1.0 / 19.0, 1.0 / 21.0, 1.0 / 23.0};
+
 __device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
 
 // exp(x) = 2^k exp(r), r = x - k ln2 (two-piece ln2), exp(r) = sum_{j<=13} r^j/j! by Horner.
@@ -20,20 +28,9 @@ __device__ __forceinline__ double exp_(double x) {
   const double kd = rint(x * LOG2E);
   double r = fma_(-kd, LN2_HI, x);
   r = fma_(-kd, LN2_LO, r);
-  double p = 1.0 / 6227020800.0;
-  p = fma_(p, r, 1.0 / 479001600.0);
-  p = fma_(p, r, 1.0 / 39916800.0);
-  p = fma_(p, r, 1.0 / 3628800.0);
-  p = fma_(p, r, 1.0 / 362880.0);
-  p = fma_(p, r, 1.0 / 40320.0);
-  p = fma_(p, r, 1.0 / 5040.0);
-  p = fma_(p, r, 1.0 / 720.0);
-  p = fma_(p, r, 1.0 / 120.0);
-  p = fma_(p, r, 1.0 / 24.0);
-  p = fma_(p, r, 1.0 / 6.0);
-  p = fma_(p, r, 1.0 / 2.0);
-  p = fma_(p, r, 1.0);
-  p = fma_(p, r, 1.0);
+  double p = EXP_C[13];
+#pragma unroll
+  for (int j = 12; j >= 0; j--) p = fma_(p, r, EXP_C[j]);
   const int k = (int)kd;  // |k| <= 1010
   const double scale = __longlong_as_double((long long)(k + 1023) << 52);
   return p * scale;  // exact: p in [0.7, 1.42], result normal
@@ -52,18 +49,9 @@ __device__ __forceinline__ double log_(double x) {
   }
   const double s = (m - 1.0) / (m + 1.0);
   const double z = s * s;
-  double p = 1.0 / 23.0;
-  p = fma_(p, z, 1.0 / 21.0);
-  p = fma_(p, z, 1.0 / 19.0);
-  p = fma_(p, z, 1.0 / 17.0);
-  p = fma_(p, z, 1.0 / 15.0);
-  p = fma_(p, z, 1.0 / 13.0);
-  p = fma_(p, z, 1.0 / 11.0);
-  p = fma_(p, z, 1.0 / 9.0);
-  p = fma_(p, z, 1.0 / 7.0);
-  p = fma_(p, z, 1.0 / 5.0);
-  p = fma_(p, z, 1.0 / 3.0);
-  p = fma_(p, z, 1.0);
+  double p = LOG_C[11];
+#pragma unroll
+  for (int j = 10; j >= 0; j--) p = fma_(p, z, LOG_C[j]);
   const double t = (2.0 * s) * p;
   const double ed = (double)e;
   return fma_(ed, LN2_HI, fma_(ed, LN2_LO, t));

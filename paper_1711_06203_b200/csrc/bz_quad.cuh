@@ -38,7 +38,9 @@ struct QuadMem {
   static constexpr int Y_OFF = S_OFF + NEQ;             // y / f gather [NEQ]
   static constexpr int U_OFF = Y_OFF + NEQ;             // pivot row broadcast, 2 x NEQ
   static constexpr int L_OFF = U_OFF + 2 * NEQ;         // lambda_k [K]
-  static constexpr int RAW = L_OFF + K;
+  static constexpr int SC_OFF = L_OFF + K;               // per-zone scalars: l[7] hs[6] rxi[6] tau[6]
+  static constexpr int SC_L = 0, SC_HS = 7, SC_RXI = 13, SC_TAU = 19, SC_N = 26;
+  static constexpr int RAW = SC_OFF + SC_N;
   static constexpr int SIZE = RAW + ((4 - (RAW % 32) + 32) % 32);  // == 4 (mod 32)
   double *base;
   __device__ __forceinline__ double &Z(int j, int i) const { return base[Z_OFF + j * NEQ + i]; }
@@ -47,6 +49,7 @@ struct QuadMem {
   __device__ __forceinline__ double *ysh() const { return base + Y_OFF; }
   __device__ __forceinline__ double *ub(int par) const { return base + U_OFF + par * NEQ; }
   __device__ __forceinline__ double *lam() const { return base + L_OFF; }
+  __device__ __forceinline__ double &sc(int i) const { return base[SC_OFF + i]; }
 };
 
 template <int NEQ>

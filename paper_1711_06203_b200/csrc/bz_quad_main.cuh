@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   double *gP = qn.gscratch + gquad * (NEQ * NEQ + 2 * NEQ);  // general path: P, b, ipvt
   const double dt = A.dt, rtol = A.rtol, atol = A.atol, fac = qn.fac;
   const double inv_n = 1.0 / (double)NEQ;
-  unsigned long long c_nst = 0, c_rhs = 0, c_jac = 0, c_lu = 0, c_sol = 0, c_etf = 0, c_cfn = 0, c_fail = 0;
+  unsigned c_nst = 0, c_rhs = 0, c_jac = 0, c_lu = 0, c_sol = 0, c_etf = 0, c_cfn = 0, c_fail = 0;  // per thread: < 2^32
 
   // component index of my slot s and its validity
 #define BZQ_I(s) (4 * (s) + c)
@@ -62,9 +62,6 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   double rho = 0.0, h = 0.0, t = 0.0, etamax = ETAMX1, hS = 0.0;
   int q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0, ncf = 0, nef = 0;
   bool newstep = true, last = false;
-  double tau[QMAX + 1];
-#pragma unroll
-  for (int i = 0; i <= QMAX; i++) tau[i] = 0.0;
   QuadLU<NEQ> lu;
 #pragma unroll
   for (int s = 0; s < S; s++) lu.invd[s] = 0.0;
@@ -143,8 +140,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             if (BZQ_OK(s)) m.Z(1, BZQ_I(s)) = h * f[s];
           q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0;
           t = 0.0, etamax = ETAMX1, hS = 0.0;
+          if (c == 0) {
 #pragma unroll
-          for (int i = 0; i <= QMAX; i++) tau[i] = 0.0;
+            for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;
+          }
           newstep = true;
           phase = 1;
         }
@@ -157,7 +156,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
 #undef BZQ_OK
 #undef BZQ_SEG_SYNC
   // ---- counters (lane 0 of each quad holds the zone's counts) ------------------------------------
-  unsigned long long cs[8] = {c_nst, c_rhs, c_jac, c_lu, c_sol, c_etf, c_cfn, c_fail};
+  const unsigned cs[8] = {c_nst, c_rhs, c_jac, c_lu, c_sol, c_etf, c_cfn, c_fail};
 #pragma unroll
   for (int k = 0; k < 8; k++) {
     unsigned long long v = (c == 0) ? cs[k] : 0ull;
