@@ -52,6 +52,32 @@ struct QuadMem {
   __device__ __forceinline__ double &sc(int i) const { return base[SC_OFF + i]; }
 };
 
+// Pascal-triangle predict / retract of one component for a compile-time order Q: no predication,
+// exactly Q+1 loads and stores (the run-time-order versions cost a select per addition).
+template <int Q, bool RETRACT, class Mem>
+__device__ __forceinline__ double nord_shift_q(const Mem &m, int i) {
+  double zc[Q + 1];
+#pragma unroll
+  for (int j = 0; j <= Q; j++) zc[j] = m.Z(j, i);
+#pragma unroll
+  for (int k = 1; k <= Q; k++)
+#pragma unroll
+    for (int j = Q; j >= k; j--) zc[j - 1] = RETRACT ? zc[j - 1] - zc[j] : zc[j - 1] + zc[j];
+#pragma unroll
+  for (int j = 0; j < Q; j++) m.Z(j, i) = zc[j];  // Z[Q] is unchanged
+  return zc[0];
+}
+template <bool RETRACT, class Mem>
+__device__ __forceinline__ double nord_shift(const Mem &m, int i, int q) {
+  switch (q) {
+    case 1: return nord_shift_q<1, RETRACT>(m, i);
+    case 2: return nord_shift_q<2, RETRACT>(m, i);
+    case 3: return nord_shift_q<3, RETRACT>(m, i);
+    case 4: return nord_shift_q<4, RETRACT>(m, i);
+    default: return nord_shift_q<5, RETRACT>(m, i);
+  }
+}
+
 template <int NEQ>
 struct QuadLU {
   static constexpr int S = (NEQ + 3) / 4;
