@@ -120,6 +120,7 @@ def run_ours(args):
     w = make_workload(cfg)                       # every rank burns its own full copy (weak scaling)
     nz, N = w.nz, w.net.nspec
     net = bz.net_create(w.net)
+    net.select_kernel(args.kernel)
     stream = torch.cuda.current_stream()
 
     # ---- device-resident arm -------------------------------------------------------------------
@@ -245,6 +246,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "coop", "tpz", "quad"],
+                    help="auto = specialised quad kernel when the topology has one, else the generic coop kernel")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

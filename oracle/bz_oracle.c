@@ -229,6 +229,13 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
 }
 
 /* ---- dense LU, LINPACK dgefa/dgesl order (step a5/a6; C.5 item 4) ------------------- */
+static unsigned long long g_interchanges = 0; /* test aid: row interchanges done by orc_lu_factor */
+unsigned long long orc_interchanges(int reset) {
+  unsigned long long v = __atomic_load_n(&g_interchanges, __ATOMIC_RELAXED);
+  if (reset) __atomic_store_n(&g_interchanges, 0ull, __ATOMIC_RELAXED);
+  return v;
+}
+
 int orc_lu_factor(int n, double *a, int32_t *ipvt, double *inv) {
   int info = 0;
   for (int k = 0; k < n; k++) {
@@ -249,6 +256,7 @@ int orc_lu_factor(int n, double *a, int32_t *ipvt, double *inv) {
       continue;
     }
     /* LINPACK: interchange rows k and p in columns k..n-1 only (earlier multipliers stay) */
+    if (p != k) __atomic_fetch_add(&g_interchanges, 1ull, __ATOMIC_RELAXED);
     if (p != k)
       for (int j = k; j < n; j++) {
         double t = a[p * n + j];
@@ -662,7 +670,7 @@ int orc_rates(const orc_net_desc *d, double rho, const double *y, double *f, dou
   if (rc) return rc;
   /* API order is (Y_0..Y_{N-1}, T); permute to the internal T-first order and back */
   const int n = nt.n, N = nt.N;
-  double yi[ORC_NMAX], fi[ORC_NMAX], Ji[ORC_NMAX * ORC_NMAX];
+  double yi[ORC_NMAX] = {0}, fi[ORC_NMAX], Ji[ORC_NMAX * ORC_NMAX];
   int ext[ORC_NMAX]; /* internal index -> external index */
   ext[TI] = N;
   for (int i = 0; i < N; i++) ext[SP(i)] = i;

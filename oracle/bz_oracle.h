@@ -69,6 +69,8 @@ void orc_lu_solve(int n, const double *a, const int32_t *ipvt, const double *inv
 void orc_bdf_coeffs(int q, double h, const double *tau, double *l);
 double orc_wrms(int n, const double *v, const double *w, int lanes);
 int orc_max_threads(void);
+/* test aid: number of row interchanges orc_lu_factor has performed since the last reset */
+unsigned long long orc_interchanges(int reset);
 
 #ifdef __cplusplus
 }

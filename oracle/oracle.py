@@ -49,6 +49,8 @@ def _L():
         lib.orc_wrms.restype = C.c_double
         lib.orc_wrms.argtypes = [C.c_int, _dp, _dp, C.c_int]
         lib.orc_max_threads.restype = C.c_int
+        lib.orc_interchanges.restype = C.c_uint64
+        lib.orc_interchanges.argtypes = [C.c_int]
         _lib = lib
     return _lib
 
@@ -77,6 +79,11 @@ def _desc(net):
               _i(keep["reactant"]), _i(keep["stoich_id"]), _d(keep["stoich_dy"]), _d(keep["rate_A"]),
               _d(keep["rate_n"]), _d(keep["rate_B"]), _d(keep["q_mev"]), float(net.cv))
     return d, keep
+
+
+def interchanges(reset: bool = False) -> int:
+    """Row interchanges performed by the LU since the last reset (test aid)."""
+    return int(_L().orc_interchanges(1 if reset else 0))
 
 
 def max_threads() -> int:

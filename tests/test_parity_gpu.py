@@ -140,3 +140,95 @@ def test_host_path_matches_device_path():
     Td, Xd, nd, *_ = _gpu_burn(w)
     assert np.array_equal(To.numpy(), Td) and np.array_equal(Xo.numpy(), Xd) and np.array_equal(ns.numpy(), nd)
     bz.net_destroy(net)
+
+
+# ---------------------------------------------------------------------------------------------
+# Full-size runs in bench.py's launch configuration (same kernel, same grid: the whole config in
+# one burn_zones call), compared on sampled zones the oracle computes one by one, plus properties
+# that hold at any size (mass invariant, valid step counts, finite outputs).
+# ---------------------------------------------------------------------------------------------
+def _full_size_check(config, sample_idx, scale=None):
+    import torch
+    import paper_1711_06203_b200 as bz
+    w = make_workload(config, zones=scale)
+    net = bz.net_create(w.net)
+    dev = torch.device("cuda:0")
+    To, Xo, ns = bz.burn_zones(net, torch.from_numpy(w.rho).to(dev), torch.from_numpy(w.T).to(dev),
+                               torch.from_numpy(w.X).to(dev), w.dt, w.rtol, w.atol)
+    torch.cuda.synchronize()
+    lanes, name = net.norm_lanes, net.kernel_name
+    To, Xo, ns = To.cpu().numpy(), Xo.cpu().numpy(), ns.cpu().numpy()
+    bz.net_destroy(net)
+    # properties at full size
+    ok = ns > 0
+    assert np.isfinite(To).all() and np.isfinite(Xo).all()
+    assert ok.mean() > 0.999
+    assert np.abs(Xo.sum(axis=0) - w.X.sum(axis=0))[ok].max() <= 1e-10
+    assert (To[ok] >= w.T[ok] * (1 - 1e-12)).all()          # exothermic forward network: T never drops
+    # sampled zones against the oracle
+    idx = np.asarray(sample_idx(w), dtype=np.int64)
+    Tr, Xr, nr, _ = oracle.burn(w.net, w.rho[idx], w.T[idx], np.ascontiguousarray(w.X[:, idx]), w.dt, w.rtol,
+                                w.atol, norm_lanes=lanes)
+    stats = compare(To[idx], Xo[:, idx], ns[idx], Tr, Xr, nr)
+    _record(f"config{config}:full", dict(stats, kernel=name, nz_gpu=int(w.nz)))
+    return w, ns
+
+
+def test_full_size_config2():
+    _full_size_check(2, lambda w: np.arange(0, w.nz, 127))
+
+
+def test_full_size_config3():
+    """BASELINE.json configs[2]: the workload bench.py times."""
+    _full_size_check(3, lambda w: np.arange(0, w.nz, 509))
+
+
+def test_full_size_config4():
+    """256^3 zones; the oracle sample holds every 64th zone with T > 1e9 and every 8191st zone."""
+    def sample(w):
+        hot = np.where(w.T > 1e9)[0]
+        return np.unique(np.concatenate([hot[::64], np.arange(0, w.nz, 8191)]))
+    w, ns = _full_size_check(4, sample)
+    assert ns.min() == 1 and ns.max() > 100                  # >100x spread in step counts
+
+
+def test_config5_eighth_size():
+    """Config 5 runs on the generic cooperative kernel (no specialised kernel yet), ~0.9 % of peak:
+    the full 128^3 grid would take ~4 min per call, so this GPU run is every 16th zone (131072 zones)."""
+    _full_size_check(5, lambda w: np.arange(0, w.nz, 97), scale=16)
+
+
+# ---------------------------------------------------------------------------------------------
+# The general LU path.  With the unknowns ordered temperature-first no config 1-4 zone ever needs
+# a row interchange, so the specialised kernels' interchange fallback (LINPACK dgefa/dgesl on a
+# scratch copy) would go untested.  Zones that start with NEGATIVE helium (and carbon) flip the
+# sign of diagonal Jacobian entries (reading s19) and do force interchanges: the oracle counts
+# them, and every kernel must still agree with it bit for bit.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["auto", "tpz", "coop"])
+@pytest.mark.parametrize("config", [2, 3])
+def test_interchange_path(config, kind):
+    net_d = network_for_config(config)
+    rng = np.random.default_rng(123 + config)
+    nz = 1536
+    rho = 10 ** rng.uniform(5, 9, nz)
+    T = rng.uniform(5e8, 3e9, nz)
+    X = np.zeros((net_d.nspec, nz))
+    X[0] = -10 ** rng.uniform(-6, -1, nz)
+    if config == 3:
+        X[1] = -10 ** rng.uniform(-6, -1, nz)
+        X[2] = 1.0 - X[0] - X[1]
+    else:
+        X[1] = 0.5
+        X[2] = 0.5 - X[0]
+    w = make_workload(config, zones=[0])
+    w.rho, w.T, w.X, w.dt = rho, T, X, 1e-6
+    To, Xo, ns, cnt, lanes, name = _gpu_burn(w, kind=kind)
+    oracle.interchanges(reset=True)
+    Tr, Xr, nr, cr = oracle.burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, norm_lanes=lanes)
+    nswap = oracle.interchanges()
+    assert nswap > 100, "the recipe no longer forces interchanges"
+    assert np.array_equal(ns, nr)
+    assert np.array_equal(To, Tr) and np.array_equal(Xo, Xr)        # bit for bit, negative X included
+    assert all(cnt[k] == cr[k] for k in cnt)
+    _record(f"interchange:config{config}:{kind}", dict(kernel=name, interchanges=nswap, nz=nz))
