@@ -57,6 +57,12 @@ __device__ __forceinline__ double log_(double x) {
   return fma_(ed, LN2_HI, fma_(ed, LN2_LO, t));
 }
 
+// x with its sign bit xor-ed by `mask` (0 or 0x80000000): a conditional negation that costs one
+// integer LOP3 on the high word instead of DADD + 2 FSEL.  Bit-identical to `cond ? -x : x`.
+__device__ __forceinline__ double flip_(double x, unsigned mask) {
+  return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
+}
+
 __device__ __forceinline__ bool finite_(double x) {
   return (__double_as_longlong(x) & 0x7ff0000000000000LL) != 0x7ff0000000000000LL;
 }
