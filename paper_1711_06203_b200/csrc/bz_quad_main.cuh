@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
 #pragma unroll
   for (int s = 0; s < S; s++) lu.invd[s] = 0.0;
 
-  for (;;) {
+  for (unsigned trip = 0;; trip++) {
     if (phase == 0) {
       // ---- a2 + a1: next zone, load, validate, initialise ------------------------------------------
       if (c == 0) z = (long long)atomicAdd(A.queue, 1ull);
@@ -149,7 +149,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
         }
       }
     }
-    if (__syncthreads_and(phase == 2)) break;
+#ifdef BZ_QUAD_BARRIER_EVERY2
+    if ((trip & 1u) == 0u)
+#endif
+      if (__syncthreads_and(phase == 2)) break;
 #include "bz_quad_attempt.inc"
   }
 #undef BZQ_I
