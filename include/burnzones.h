@@ -73,7 +73,7 @@ int net_create(const bz_net_desc *desc, bz_net **out);
  *   nsteps         DEVICE [nz] int32: accepted BDF steps, or a per-zone failure code
  *                    -1  more than 10 Newton failures on one step
  *                    -2  7 error-test failures on one step
- *                    -3  100000 steps taken without reaching dt
+ *                    -3  20000 steps taken without reaching dt
  *                    -4  invalid input zone (non-finite, rho <= 0 or T <= 0): outputs = inputs
  *                  failed zones hold the last accepted state; they do not fail the call.
  *   cuda_stream    cudaStream_t (as void*) on which all work is enqueued

@@ -35,7 +35,7 @@
 #define ETAMXF 0.2
 #define ETAMX1 1e4
 #define ETAMAX 2.0
-#define MXSTEP 100000
+#define MXSTEP 20000
 #define SLIVER 1e-6
 
 static const double FACT[8] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0, 720.0, 5040.0};

@@ -22,7 +22,7 @@
 namespace bz {
 
 // ---- constants of BZ-BDF v1 ---------------------------------------------------
-constexpr int QMAX = 5, MAXCOR = 3, MXNCF = 10, MXNEF = 7, MXSTEP = 100000;
+constexpr int QMAX = 5, MAXCOR = 3, MXNCF = 10, MXNEF = 7, MXSTEP = 20000;
 constexpr double NTOL = 0.1, CRDOWN = 0.3, RDIV = 2.0, ETACF = 0.25;
 constexpr double BIAS1 = 4.0, BIAS2 = 6.0, BIAS3 = 10.0, ADDON = 1e-6, THRESH = 1.5;
 constexpr double ETAMIN = 0.1, ETAMXF = 0.2, ETAMX1 = 1e4, ETAMAX = 2.0, SLIVER = 1e-6;
