@@ -87,10 +87,8 @@ QuadVariant make_quad(const char *name) {
 // measured 1.8x faster, profiles/README.md).  BZ_QUAD_SHAPE=128x3|384x1 picks one at net_create.
 #define BZ_QUAD_ENTRY3(NET) make_quad<NET, 128, 3>("burn_quad<" #NET ",128x3>"),
 #define BZ_QUAD_ENTRY2(NET) make_quad<NET, 384, 1>("burn_quad<" #NET ",384x1>"),
-#define BZ_QUAD_ENTRY1(NET) make_quad<NET, 192, 2>("burn_quad<" #NET ",192x2>"),
 const QuadVariant kQuad3[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY3)};
 const QuadVariant kQuad2[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY2)};
-const QuadVariant kQuad1[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY1)};
 
 #define BZ_TPZ_ENTRY(NET) make_tpz<NET>("burn_tpz<" #NET ">"),
 const TpzVariant kTpz[] = {BZ_TPZ_NETS(BZ_TPZ_ENTRY)};
@@ -325,7 +323,6 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     const QuadVariant *tab = kQuad2;  // default: 384x1
     if (const char *e = std::getenv("BZ_QUAD_SHAPE")) {
       if (!std::strcmp(e, "128x3")) tab = kQuad3;
-      if (!std::strcmp(e, "192x2")) tab = kQuad1;
     }
     const int ntab = (int)(sizeof(kQuad3) / sizeof(kQuad3[0]));
     for (int i = 0; i < ntab; i++)
