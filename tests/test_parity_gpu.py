@@ -232,3 +232,75 @@ def test_interchange_path(config, kind):
     assert np.array_equal(To, Tr) and np.array_equal(Xo, Xr)        # bit for bit, negative X included
     assert all(cnt[k] == cr[k] for k in cnt)
     _record(f"interchange:config{config}:{kind}", dict(kernel=name, interchanges=nswap, nz=nz))
+
+
+# ---------------------------------------------------------------------------------------------
+# Generic networks of other sizes: they run on the cooperative kernel's PADDED instances
+# (n rounded up to 4/8/16/32 lanes with identity rows), which no config exercises, and at the
+# ABI's maximum sizes (31 species, 256 reactions).
+# ---------------------------------------------------------------------------------------------
+def _random_network(nspec, nreac, seed):
+    from workloads.configs import Network
+    rng = np.random.default_rng(seed)
+    reactant = -np.ones((nreac, 3), dtype=np.int32)
+    sid = -np.ones((nreac, 4), dtype=np.int32)
+    sdy = np.zeros((nreac, 4))
+    aion = 4.0 * (np.arange(nspec) + 1.0)
+    for k in range(nreac):
+        kind = rng.integers(0, 4) if nspec > 2 else rng.integers(0, 2)
+        if kind == 0:                                  # decay  i -> j
+            i, j = rng.choice(nspec, 2, replace=False)
+            reactant[k, 0] = i
+            sid[k, :2] = (i, j)
+            sdy[k, :2] = (-1.0, aion[i] / aion[j])
+        elif kind == 1:                                # pair   i + i -> j
+            i, j = rng.choice(nspec, 2, replace=False)
+            reactant[k, :2] = (i, i)
+            sid[k, :2] = (i, j)
+            sdy[k, :2] = (-2.0, 2 * aion[i] / aion[j])
+        elif kind == 2:                                # capture i + j -> l
+            i, j, l = rng.choice(nspec, 3, replace=False)
+            reactant[k, :2] = (i, j)
+            sid[k, :3] = (i, j, l)
+            sdy[k, :3] = (-1.0, -1.0, (aion[i] + aion[j]) / aion[l])
+        else:                                          # triple i + i + i -> j
+            i, j = rng.choice(nspec, 2, replace=False)
+            reactant[k] = (i, i, i)
+            sid[k, :2] = (i, j)
+            sdy[k, :2] = (-3.0, 3 * aion[i] / aion[j])
+    A = 10.0 ** rng.uniform(3, 12, nreac)
+    return Network(f"rand{nspec}x{nreac}", [f"s{i}" for i in range(nspec)], aion, reactant, sid, sdy,
+                   A, rng.uniform(-1, 1, nreac), rng.uniform(5, 40, nreac), rng.uniform(-2, 8, nreac))
+
+
+@pytest.mark.parametrize("nspec,nreac,nz", [(1, 1, 40), (3, 4, 300), (5, 9, 300), (9, 20, 200), (15, 40, 150),
+                                            (20, 60, 100), (31, 256, 48)])
+def test_generic_network_sizes(nspec, nreac, nz):
+    import torch
+    import paper_1711_06203_b200 as bz
+    if nspec == 1:
+        from workloads.configs import Network
+        net_d = Network("one", ["s0"], np.array([4.0]), np.array([[0, -1, -1]], dtype=np.int32),
+                        np.array([[0, -1, -1, -1]], dtype=np.int32), np.array([[-1.0, 0, 0, 0]]),
+                        np.array([3e6]), np.array([0.5]), np.array([2.0]), np.array([1.5]))
+    else:
+        net_d = _random_network(nspec, nreac, seed=1000 + nspec)
+    rng = np.random.default_rng(nspec)
+    rho = 10 ** rng.uniform(4, 7, nz)
+    T = rng.uniform(8e8, 3e9, nz)
+    X = rng.random((nspec, nz)) + 0.01
+    X /= X.sum(axis=0)
+    net = bz.net_create(net_d)
+    assert net.kernel_name.startswith("burn_coop")
+    dev = torch.device("cuda:0")
+    To, Xo, ns = bz.burn_zones(net, torch.from_numpy(rho).to(dev), torch.from_numpy(T).to(dev),
+                               torch.from_numpy(X).to(dev), 1e-6, 1e-8, 1e-12)
+    torch.cuda.synchronize()
+    cnt = bz.get_counters(net)
+    Tr, Xr, nr, cr = oracle.burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, norm_lanes=net.norm_lanes)
+    stats = compare(To.cpu().numpy(), Xo.cpu().numpy(), ns.cpu().numpy(), Tr, Xr, nr)
+    assert stats["nsteps_equal"] == 1.0 and stats["bitexact_X"] == 1.0 and stats["bitexact_T"] == 1.0
+    assert all(cnt[k] == cr[k] for k in cnt)
+    assert (nr > 1).mean() > 0.5                     # the networks are alive: real multi-step burns
+    _record(f"generic:{nspec}x{nreac}", dict(stats, kernel=net.kernel_name))
+    bz.net_destroy(net)
