@@ -229,10 +229,20 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
 }
 
 /* ---- dense LU, LINPACK dgefa/dgesl order (step a5/a6; C.5 item 4) ------------------- */
-static unsigned long long g_interchanges = 0; /* test aid: row interchanges done by orc_lu_factor */
+/* test aids: how often rarely taken paths ran since the last reset --
+ * [0] row interchanges in orc_lu_factor, [1] third error-test failure lowering the order
+ * (C.2-B.5, q > 1), [2] third error-test failure restarting at order 1 (q = 1). */
+static unsigned long long g_events[3] = {0, 0, 0};
+#define ORC_EVENT(i) __atomic_fetch_add(&g_events[i], 1ull, __ATOMIC_RELAXED)
+void orc_event_counts(int reset, unsigned long long out[3]) {
+  for (int i = 0; i < 3; i++) {
+    out[i] = __atomic_load_n(&g_events[i], __ATOMIC_RELAXED);
+    if (reset) __atomic_store_n(&g_events[i], 0ull, __ATOMIC_RELAXED);
+  }
+}
 unsigned long long orc_interchanges(int reset) {
-  unsigned long long v = __atomic_load_n(&g_interchanges, __ATOMIC_RELAXED);
-  if (reset) __atomic_store_n(&g_interchanges, 0ull, __ATOMIC_RELAXED);
+  unsigned long long v = __atomic_load_n(&g_events[0], __ATOMIC_RELAXED);
+  if (reset) __atomic_store_n(&g_events[0], 0ull, __ATOMIC_RELAXED);
   return v;
 }
 
@@ -256,7 +266,7 @@ int orc_lu_factor(int n, double *a, int32_t *ipvt, double *inv) {
       continue;
     }
     /* LINPACK: interchange rows k and p in columns k..n-1 only (earlier multipliers stay) */
-    if (p != k) __atomic_fetch_add(&g_interchanges, 1ull, __ATOMIC_RELAXED);
+    if (p != k) ORC_EVENT(0);
     if (p != k)
       for (int j = k; j < n; j++) {
         double t = a[p * n + j];
@@ -519,6 +529,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
         rescale(n, q, Z, eta);
         h = h * eta;
       } else if (q > 1) {
+        ORC_EVENT(1);
         /* lower the order at t_{n-1}: xi_i = (tau_1 + ... + tau_i)/h */
         double s = 0.0;
         for (int i = 1; i <= q - 2; i++) {
@@ -533,6 +544,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
         rescale(n, q, Z, ETAMIN);
         h = h * ETAMIN;
       } else {
+        ORC_EVENT(2);
         h = h * ETAMIN;
         for (int i = 0; i < n; i++) y[i] = Z[0][i];
         rates(nt, rho, y, f, NULL);

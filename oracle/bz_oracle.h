@@ -71,6 +71,8 @@ double orc_wrms(int n, const double *v, const double *w, int lanes);
 int orc_max_threads(void);
 /* test aid: number of row interchanges orc_lu_factor has performed since the last reset */
 unsigned long long orc_interchanges(int reset);
+/* test aid: {interchanges, order lowered after a 3rd error-test failure, order-1 restart} */
+void orc_event_counts(int reset, unsigned long long out[3]);
 
 #ifdef __cplusplus
 }

@@ -49,6 +49,8 @@ def _L():
         lib.orc_wrms.restype = C.c_double
         lib.orc_wrms.argtypes = [C.c_int, _dp, _dp, C.c_int]
         lib.orc_max_threads.restype = C.c_int
+        lib.orc_event_counts.restype = None
+        lib.orc_event_counts.argtypes = [C.c_int, C.POINTER(C.c_uint64)]
         lib.orc_interchanges.restype = C.c_uint64
         lib.orc_interchanges.argtypes = [C.c_int]
         _lib = lib
@@ -84,6 +86,13 @@ def _desc(net):
 def interchanges(reset: bool = False) -> int:
     """Row interchanges performed by the LU since the last reset (test aid)."""
     return int(_L().orc_interchanges(1 if reset else 0))
+
+
+def event_counts(reset: bool = False) -> dict:
+    """How often rarely taken paths ran since the last reset (test aid)."""
+    out = (C.c_uint64 * 3)()
+    _L().orc_event_counts(1 if reset else 0, out)
+    return dict(interchanges=int(out[0]), etf_lower_order=int(out[1]), etf_restart_order1=int(out[2]))
 
 
 def max_threads() -> int:

@@ -304,3 +304,33 @@ def test_generic_network_sizes(nspec, nreac, nz):
     assert (nr > 1).mean() > 0.5                     # the networks are alive: real multi-step burns
     _record(f"generic:{nspec}x{nreac}", dict(stats, kernel=net.kernel_name))
     bz.net_destroy(net)
+
+
+# ---------------------------------------------------------------------------------------------
+# Stress inputs: negative abundances, T up to 8e9 K, rho up to 3e10, dt up to 1e-3 s.  They make
+# the integrator take paths no config takes -- Newton failures (B.6) and the order reduction after
+# a third error-test failure (B.5) -- on the specialised kernels as well as on the generic one.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["auto", "tpz", "coop"])
+@pytest.mark.parametrize("trial", [2, 3])
+def test_stress_inputs_config3_topology(trial, kind):
+    net_d = network_for_config(3)
+    dt, neglo, neghi, Tlo, Thi, rlo, rhi = [(1e-3, -2, -0.3, 2e9, 6e9, 7, 10), (1e-5, -1, -0.1, 3e9, 8e9, 8, 10.5)][trial - 2]
+    rng = np.random.default_rng(50 + trial)
+    nz = 2048
+    rho = 10 ** rng.uniform(rlo, rhi, nz)
+    T = rng.uniform(Tlo, Thi, nz)
+    X = np.zeros((net_d.nspec, nz))
+    X[0] = -10 ** rng.uniform(neglo, neghi, nz)
+    X[1] = rng.uniform(-0.2, 0.6, nz)
+    X[2] = 1 - X[0] - X[1]
+    w = make_workload(3, zones=[0])
+    w.rho, w.T, w.X, w.dt = rho, T, X, dt
+    To, Xo, ns, cnt, lanes, name = _gpu_burn(w, kind=kind)
+    oracle.event_counts(reset=True)
+    Tr, Xr, nr, cr = oracle.burn(net_d, rho, T, X, dt, 1e-8, 1e-12, norm_lanes=lanes)
+    ev = oracle.event_counts()
+    assert cr["ncfn"] > 0 and ev["etf_lower_order"] > 0, (cr, ev)
+    assert np.array_equal(ns, nr) and np.array_equal(To, Tr) and np.array_equal(Xo, Xr)
+    assert all(cnt[k] == cr[k] for k in cnt)
+    _record(f"stress:trial{trial}:{kind}", dict(kernel=name, ncfn=cr["ncfn"], netf=cr["netf"], **ev))
