@@ -1,4 +1,4 @@
-// bz_quad.cuh -- 4 lanes per zone ("quad") burn kernel pieces, DESIGN.md section 5.3.
+// bz_quad.cuh -- 4 lanes per zone ("quad") burn kernel pieces, DESIGN.md section 5.4.
 //
 // Why 4 lanes: a zone's integrator state is ~3 KB (n = 14: P/LU 196, Z 84, vectors ~60 doubles),
 // so only ~100-130 zones fit on an SM.  One thread per zone then means 3-4 warps per SM and every
@@ -95,8 +95,6 @@ struct QuadLU {
     bool swap_needed = false, bad = false;
 #pragma unroll
     for (int k = 0; k < NEQ; k++) {
-      constexpr int dummy = 0;
-      (void)dummy;
       const int ko = k & 3, ks = k >> 2;
       double *ub = m.ub(k & 1);
       if (c == ko) {
