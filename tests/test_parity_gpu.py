@@ -334,3 +334,28 @@ def test_stress_inputs_config3_topology(trial, kind):
     assert np.array_equal(ns, nr) and np.array_equal(To, Tr) and np.array_equal(Xo, Xr)
     assert all(cnt[k] == cr[k] for k in cnt)
     _record(f"stress:trial{trial}:{kind}", dict(kernel=name, ncfn=cr["ncfn"], netf=cr["netf"], **ev))
+
+
+def test_repeatable_and_stream_ordered():
+    """compute-sanitizer is closed on this pool, so races are hunted by repetition: the same burn,
+    five times, on a side stream with the outputs of run k feeding nothing -- all bit-identical
+    (the work queue hands zones to groups in a different order every time)."""
+    import torch
+    import paper_1711_06203_b200 as bz
+    w = make_workload(3, zones=1021)
+    dev = torch.device("cuda:0")
+    rho, T, X = (torch.from_numpy(a).to(dev) for a in (w.rho, w.T, w.X))
+    for kind in ("auto", "tpz", "coop"):
+        net = bz.net_create(w.net)
+        net.select_kernel(kind)
+        side = torch.cuda.Stream()
+        outs = []
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            for _ in range(5):
+                To, Xo, ns = bz.burn_zones(net, rho, T, X, w.dt, w.rtol, w.atol, stream=side)
+                outs.append((To, Xo, ns))
+        side.synchronize()
+        for To, Xo, ns in outs[1:]:
+            assert torch.equal(To, outs[0][0]) and torch.equal(Xo, outs[0][1]) and torch.equal(ns, outs[0][2])
+        bz.net_destroy(net)
