@@ -36,8 +36,8 @@ struct QuadMem {
   static constexpr int W_OFF = Z_OFF + (QMAX + 1) * NEQ; // w[NEQ]
   static constexpr int S_OFF = W_OFF + NEQ;             // saved vector S[NEQ]
   static constexpr int Y_OFF = S_OFF + NEQ;             // y / f gather [NEQ]
-  static constexpr int U_OFF = Y_OFF + NEQ;             // pivot row broadcast, 2 x NEQ
-  static constexpr int L_OFF = U_OFF + 2 * NEQ;         // lambda_k [K]
+  static constexpr int U_OFF = Y_OFF + NEQ;             // pivot row broadcast, 2 x (NEQ + 1)
+  static constexpr int L_OFF = U_OFF + 2 * (NEQ + 1);   // lambda_k [K]
   static constexpr int SC_OFF = L_OFF + K;               // per-zone scalars: l[7] hs[6] rxi[6] tau[6]
   static constexpr int SC_L = 0, SC_HS = 7, SC_RXI = 13, SC_TAU = 19, SC_N = 26;
   static constexpr int RAW = SC_OFF + SC_N;
@@ -47,7 +47,7 @@ struct QuadMem {
   __device__ __forceinline__ double &W(int i) const { return base[W_OFF + i]; }
   __device__ __forceinline__ double &Sv(int i) const { return base[S_OFF + i]; }
   __device__ __forceinline__ double *ysh() const { return base + Y_OFF; }
-  __device__ __forceinline__ double *ub(int par) const { return base + U_OFF + par * NEQ; }
+  __device__ __forceinline__ double *ub(int par) const { return base + U_OFF + par * (NEQ + 1); }  // row + its b
   __device__ __forceinline__ double *lam() const { return base + L_OFF; }
   __device__ __forceinline__ double &sc(int i) const { return base[SC_OFF + i]; }
 };
@@ -90,8 +90,10 @@ struct QuadLU {
 
   // no-interchange factorisation.  returns bit 0: an interchange was needed (results invalid),
   // bit 1: zero / NaN pivot.  Quad-uniform result.
+  // b: right-hand side of the first solve; its forward elimination (dgesl, k ascending) rides along:
+  // the pivot row's b_k is published with the row, so the first solve needs only back_solve().
   template <class Mem>
-  __device__ __forceinline__ unsigned factor(const Mem &m, int c, unsigned gmask) {
+  __device__ __forceinline__ unsigned factor(const Mem &m, int c, unsigned gmask, double (&b)[S]) {
     bool swap_needed = false, bad = false;
 #pragma unroll
     for (int k = 0; k < NEQ; k++) {
@@ -100,9 +102,11 @@ struct QuadLU {
       if (c == ko) {
 #pragma unroll
         for (int j = k; j < NEQ; j++) ub[j] = a[ks][j];
+        ub[NEQ] = b[ks];
       }
       __syncwarp(gmask);
       const double piv = ub[k];
+      const double bk = ub[NEQ];
       const unsigned hk = hi_abs(piv);
       bad |= !(fabs(piv) > 0.0);
       const double inv = 1.0 / piv;
@@ -118,6 +122,7 @@ struct QuadLU {
           a[s][k] = l;
 #pragma unroll
           for (int j = k + 1; j < NEQ; j++) a[s][j] = fma_(-l, ub[j], a[s][j]);
+          b[s] = fma_(-l, bk, b[s]);
         }
       }
     }
@@ -141,6 +146,10 @@ struct QuadLU {
         if ((s > ks) || (c > ko)) b[s] = fma_(-a[s][k], bk, b[s]);
       }
     }
+    back_solve(c, gmask, b);
+  }
+  // backward half only (the forward half was fused into factor())
+  __device__ __forceinline__ void back_solve(int c, unsigned gmask, double (&b)[S]) const {
 #pragma unroll
     for (int k = NEQ - 1; k >= 0; k--) {
       const int ko = k & 3, ks = k >> 2;
