@@ -39,8 +39,13 @@ struct QuadMem {
   static constexpr int U_OFF = Y_OFF + NEQ;             // pivot row broadcast, 2 x (NEQ + 1)
   static constexpr int L_OFF = U_OFF + 2 * (NEQ + 1);   // lambda_k [K]
   static constexpr int SC_OFF = L_OFF + K;               // per-zone scalars: l[7] hs[6] rxi[6] tau[6]
-  static constexpr int SC_L = 0, SC_HS = 7, SC_RXI = 13, SC_TAU = 19, SC_N = 26;
-  static constexpr int RAW = SC_OFF + SC_N;
+  static constexpr int SC_L = 0, SC_HS = 7, SC_RXI = 13, SC_TAU = 19;
+  // rarely used per-zone scalars, parked here instead of in registers (every lane of the quad
+  // stores the same bits and reads them back: no intra-quad synchronisation needed)
+  static constexpr int SC_T = 26, SC_ETAMAX = 27, SC_HSAV = 28, SC_ZID = 29, SC_INT = 30, SC_N = 31;
+  static constexpr int CNT_OFF = SC_OFF + SC_N;         // event counters of this quad: 8 x uint32 (lane 0 only)
+  static constexpr int CN_NST = 0, CN_XRHS = 1, CN_INIT = 2, CN_LU = 3, CN_SOL = 4, CN_ETF = 5, CN_CFN = 6, CN_FAIL = 7;
+  static constexpr int RAW = CNT_OFF + 4;
   static constexpr int SIZE = RAW + ((4 - (RAW % 32) + 32) % 32);  // == 4 (mod 32)
   double *base;
   __device__ __forceinline__ double &Z(int j, int i) const { return base[Z_OFF + j * NEQ + i]; }
@@ -50,6 +55,9 @@ struct QuadMem {
   __device__ __forceinline__ double *ub(int par) const { return base + U_OFF + par * (NEQ + 1); }  // row + its b
   __device__ __forceinline__ double *lam() const { return base + L_OFF; }
   __device__ __forceinline__ double &sc(int i) const { return base[SC_OFF + i]; }
+  __device__ __forceinline__ long long &zid() const { return *reinterpret_cast<long long *>(base + SC_OFF + SC_ZID); }
+  __device__ __forceinline__ int &isc(int i) const { return reinterpret_cast<int *>(base + SC_OFF + SC_INT)[i]; }  // 0: qS, 1: ntau
+  __device__ __forceinline__ unsigned &cnt(int i) const { return reinterpret_cast<unsigned *>(base + CNT_OFF)[i]; }
 };
 
 // Pascal-triangle predict / retract of one component for a compile-time order Q: no predication,
@@ -81,44 +89,55 @@ __device__ __forceinline__ double nord_shift(const Mem &m, int i, int q) {
 template <int NEQ>
 struct QuadLU {
   static constexpr int S = (NEQ + 3) / 4;
-  double a[S][NEQ];  // my rows of P, then of its LU factors (l_ik below the diagonal, U above)
-  double invd[S];    // 1/pivot of my rows
+  double a[S][NEQ];  // my rows of P, then of its LU factors: l_ik below the diagonal, U above it,
+                     // 1/pivot ON the diagonal (LINPACK keeps the pivot; only its reciprocal is used)
 
   __device__ __forceinline__ static unsigned hi_abs(double x) {
     return (unsigned)(__double_as_longlong(x) >> 32) & 0x7fffffffu;
   }
 
-  // no-interchange factorisation.  returns bit 0: an interchange was needed (results invalid),
-  // bit 1: zero / NaN pivot.  Quad-uniform result.
+  // no-interchange factorisation.  returns bit 0: an interchange may be needed (results invalid,
+  // redo on the general path), bit 1: zero / NaN pivot.  Quad-uniform result.
+  // Interchange test: LINPACK swaps iff some |a_ik| > |a_kk| below the diagonal, i.e. iff the exact
+  // quotient exceeds 1 in magnitude.  The computed multiplier l = RN(a_ik * RN(1/a_kk)) is within
+  // 2 ulp of that quotient, so |l| < 1 - 2^-21 (high word below 0x3FEFFFFF) proves that no swap is
+  // needed; anything else (near-ties, exact ties, NaN) takes the general path, which pivots exactly.
+  // Cost: one AND and one unsigned max per multiplier instead of a compare-and-select chain.
   // b: right-hand side of the first solve; its forward elimination (dgesl, k ascending) rides along:
   // the pivot row's b_k is published with the row, so the first solve needs only back_solve().
   template <class Mem>
   __device__ __forceinline__ unsigned factor(const Mem &m, int c, unsigned gmask, double (&b)[S]) {
-    bool swap_needed = false, bad = false;
+    unsigned lmax = 0u;
+    bool bad = false;
 #pragma unroll
     for (int k = 0; k < NEQ; k++) {
       const int ko = k & 3, ks = k >> 2;
       double *ub = m.ub(k & 1);
       if (c == ko) {
+#ifndef BZ_QUAD_ROW_STS128
+        volatile double *vb = ub;  // 64-bit stores straight from the row's registers (no tuple packing)
+#pragma unroll
+        for (int j = k; j < NEQ; j++) vb[j] = a[ks][j];
+        vb[NEQ] = b[ks];
+#else
 #pragma unroll
         for (int j = k; j < NEQ; j++) ub[j] = a[ks][j];
         ub[NEQ] = b[ks];
+#endif
       }
       __syncwarp(gmask);
       const double piv = ub[k];
       const double bk = ub[NEQ];
-      const unsigned hk = hi_abs(piv);
       bad |= !(fabs(piv) > 0.0);
       const double inv = 1.0 / piv;
-      if (c == ko) invd[ks] = inv;
+      if (c == ko) a[ks][k] = inv;
 #pragma unroll
       for (int s = 0; s < S; s++) {
         if (s < ks) continue;
         const bool mine = (s > ks) || (c > ko);  // row 4s+c is below the pivot row
         if (mine) {
-          const double v = a[s][k];
-          if (hi_abs(v) >= hk) swap_needed |= (fabs(v) > fabs(piv));
-          const double l = v * inv;
+          const double l = a[s][k] * inv;
+          lmax = max(lmax, hi_abs(l));
           a[s][k] = l;
 #pragma unroll
           for (int j = k + 1; j < NEQ; j++) a[s][j] = fma_(-l, ub[j], a[s][j]);
@@ -126,7 +145,7 @@ struct QuadLU {
         }
       }
     }
-    const unsigned f = (swap_needed ? 1u : 0u) | (bad ? 2u : 0u);
+    const unsigned f = (lmax >= 0x3FEFFFFFu ? 1u : 0u) | (bad ? 2u : 0u);
     // make the flags quad-uniform
     unsigned r = f;
     r |= __shfl_xor_sync(gmask, r, 1, 4);
@@ -153,7 +172,7 @@ struct QuadLU {
 #pragma unroll
     for (int k = NEQ - 1; k >= 0; k--) {
       const int ko = k & 3, ks = k >> 2;
-      const double x = b[ks] * invd[ks];
+      const double x = b[ks] * a[ks][k];  // lane ko: its 1/pivot (other lanes' x is unused)
       if (c == ko) b[ks] = x;
       const double xk = __shfl_sync(gmask, x, ko, 4);
 #pragma unroll

@@ -22,12 +22,26 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   const int c = threadIdx.x & 3;
   const unsigned gmask = 0xfu << ((threadIdx.x & 31) & ~3);
   Mem m;
+#ifdef BZ_QUAD_OPAQUE_BASE
+  {
+    int zoff = ((4 * K + N + 1) & ~1) + (threadIdx.x >> 2) * Mem::SIZE;
+    asm volatile("" : "+r"(zoff));  // opaque: kept in a register instead of being recomputed from %tid at every use
+    m.base = smem + zoff;
+  }
+#else
   m.base = smem + ((4 * K + N + 1) & ~1) + (threadIdx.x >> 2) * Mem::SIZE;
+#endif
   const long long gquad = (long long)blockIdx.x * (QUAD_THREADS / 4) + (threadIdx.x >> 2);
   double *gP = qn.gscratch + gquad * (NEQ * NEQ + 2 * NEQ);  // general path: P, b, ipvt
   const double dt = A.dt, rtol = A.rtol, atol = A.atol, fac = qn.fac;
   const double inv_n = 1.0 / (double)NEQ;
-  unsigned c_nst = 0, c_rhs = 0, c_jac = 0, c_lu = 0, c_sol = 0, c_etf = 0, c_cfn = 0, c_fail = 0;  // per thread: < 2^32
+  // event counters live in the quad's shared memory (lane 0 counts): registers are the scarce
+  // resource of this kernel.  nrhs = nlu + ninit + xrhs and njac = nlu + ninit are derived at the end.
+#define BZQ_COUNT(k) do { if (c == 0) m.cnt(Mem::k) += 1u; } while (0)
+  if (c == 0) {
+#pragma unroll
+    for (int k = 0; k < 8; k++) m.cnt(k) = 0u;
+  }
 
   // component index of my slot s and its validity
 #define BZQ_I(s) (4 * (s) + c)
@@ -56,21 +70,41 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
     return sqrt(qsum(p) * inv_n);
   };
   auto qany = [&](bool p) { return (__ballot_sync(gmask, p) & gmask) != 0u; };
+  // full-warp versions for the warp-uniform part of an attempt (constant mask: no mask matching)
+  constexpr unsigned FULLMASK = 0xffffffffu;
+  auto qanyw = [&](bool p) { return (__ballot_sync(FULLMASK, p) & gmask) != 0u; };
+  auto wrmsw = [&](const double (&v)[S]) {
+    double p = 0.0;
+#pragma unroll
+    for (int s = 0; s < S; s++)
+      if (BZQ_OK(s)) {
+        const double d = v[s] * m.W(BZQ_I(s));
+        p = fma_(d, d, p);
+      }
+    p = p + __shfl_xor_sync(FULLMASK, p, 2, 4);
+    p = p + __shfl_xor_sync(FULLMASK, p, 1, 4);
+    return sqrt(p * inv_n);
+  };
 
   int phase = 0;  // 0 need a zone, 1 stepping, 2 queue empty
-  long long z = 0;
-  double rho = 0.0, h = 0.0, t = 0.0, etamax = ETAMX1, hS = 0.0;
-  int q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0, ncf = 0, nef = 0;
+  double rho = 0.0, h = 0.0;
+  int q = 1, nqwait = 2, nst = 0, ncf = 0, nef = 0;
+  // t, etamax, h_S, q_S, ntau and the zone index live in the zone's shared memory (bz_quad.cuh)
+#define BZQ_T m.sc(Mem::SC_T)
+#define BZQ_ETAMAX m.sc(Mem::SC_ETAMAX)
+#define BZQ_HSAV m.sc(Mem::SC_HSAV)
+#define BZQ_QS m.isc(0)
+#define BZQ_NTAU m.isc(1)
   bool newstep = true, last = false;
   QuadLU<NEQ> lu;
-#pragma unroll
-  for (int s = 0; s < S; s++) lu.invd[s] = 0.0;
 
   for (unsigned trip = 0;; trip++) {
     if (phase == 0) {
       // ---- a2 + a1: next zone, load, validate, initialise ------------------------------------------
+      long long z = 0;
       if (c == 0) z = (long long)atomicAdd(A.queue, 1ull);
       z = __shfl_sync(gmask, z, 0, 4);
+      m.zid() = z;
       if (z >= A.nz) {
         phase = 2;
       } else {
@@ -102,7 +136,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             } else if (i < NEQ)
               A.X_out[(long long)(i - 1) * A.nz + z] = xin[s];
           }
-          c_fail++;
+          BZQ_COUNT(CN_FAIL);
         } else {
           double f[S], v[S];
           __syncwarp(gmask);
@@ -115,7 +149,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             }
           __syncwarp(gmask);
           Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, f, lu.a);
-          c_rhs++, c_jac++;
+          BZQ_COUNT(CN_INIT);
           // exact second derivative y'' = J f for the first step size
           __syncwarp(gmask);
 #pragma unroll
@@ -138,8 +172,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
 #pragma unroll
           for (int s = 0; s < S; s++)
             if (BZQ_OK(s)) m.Z(1, BZQ_I(s)) = h * f[s];
-          q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0;
-          t = 0.0, etamax = ETAMX1, hS = 0.0;
+          q = 1, nqwait = 2, nst = 0;
+          BZQ_QS = 0, BZQ_NTAU = 0;
+          BZQ_T = 0.0, BZQ_ETAMAX = ETAMX1, BZQ_HSAV = 0.0;
           if (c == 0) {
 #pragma unroll
             for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;
@@ -159,7 +194,18 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
 #undef BZQ_OK
 #undef BZQ_SEG_SYNC
   // ---- counters (lane 0 of each quad holds the zone's counts) ------------------------------------
-  const unsigned cs[8] = {c_nst, c_rhs, c_jac, c_lu, c_sol, c_etf, c_cfn, c_fail};
+#undef BZQ_COUNT
+#undef BZQ_T
+#undef BZQ_ETAMAX
+#undef BZQ_HSAV
+#undef BZQ_QS
+#undef BZQ_NTAU
+  unsigned long long cs[8];
+  {
+    const unsigned long long lu_ = m.cnt(Mem::CN_LU), in_ = m.cnt(Mem::CN_INIT);
+    cs[0] = m.cnt(Mem::CN_NST), cs[1] = lu_ + in_ + m.cnt(Mem::CN_XRHS), cs[2] = lu_ + in_, cs[3] = lu_;
+    cs[4] = m.cnt(Mem::CN_SOL), cs[5] = m.cnt(Mem::CN_ETF), cs[6] = m.cnt(Mem::CN_CFN), cs[7] = m.cnt(Mem::CN_FAIL);
+  }
 #pragma unroll
   for (int k = 0; k < 8; k++) {
     unsigned long long v = (c == 0) ? cs[k] : 0ull;
