@@ -40,7 +40,8 @@ typedef enum {
                           coefficient, reaction without reactant, repeated stoichiometry id    */
   BZ_ERR_SCALAR = -4,  /* dt <= 0, rtol <= 0, atol < 0, or non-finite                         */
   BZ_ERR_CUDA = -5,    /* CUDA runtime error; the cudaError_t is in bz_last_cuda_error()      */
-  BZ_ERR_NOMEM = -6    /* host or device allocation failed                                    */
+  BZ_ERR_NOMEM = -6,   /* host or device allocation failed                                    */
+  BZ_ERR_UNSUPPORTED = -7 /* the kernel forced with bz_select_kernel cannot do what was asked     */
 } bz_status;
 
 /* Network descriptor.  All pointers are HOST pointers and are
@@ -83,6 +84,22 @@ int net_create(const bz_net_desc *desc, bz_net **out);
 int burn_zones(const bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
                double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
                void *cuda_stream);
+
+/* The burn with constant per-zone source terms: the coupling the paper's codes use when the burn is
+ * driven by an SDC hydro update ("SDC ... coupling of hydro and reactions", section
+ * 3.2): the advective source is held constant over the burn and the system integrated is
+ *     dT/dt = f_T(rho, y) + src_T[z],      dY_i/dt = f_i(rho, y) + src_X[i][z] / A_i .
+ *   src_T   DEVICE [nz]     temperature source, K/s
+ *   src_X   DEVICE [N][nz]  mass-fraction sources, 1/s (species-major like X)
+ * Both NULL: identical to burn_zones (bit for bit).  Exactly one NULL: BZ_ERR_NULL.  The sources
+ * enter every right-hand-side evaluation as one rounded addition after the network's own sums;
+ * the Jacobian is unchanged.  A zone with a non-finite source ends with code -4.  All other
+ * arguments, the failure codes and the execution rules are those of burn_zones.  Served by the
+ * cooperative and the quad kernels; with the thread-per-zone kernel forced (bz_select_kernel
+ * kind 2) the call returns BZ_ERR_UNSUPPORTED.  (DESIGN.md section 10.) */
+int burn_zones_src(const bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
+                   const double *src_T, const double *src_X, double dt, double rtol, double atol,
+                   double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream);
 
 /* The same burn with HOST arrays (pinned memory recommended): copies inputs to library-owned
  * device staging, runs burn_zones, copies the three outputs back, all on `cuda_stream`, and

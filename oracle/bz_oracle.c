@@ -384,9 +384,16 @@ static void rescale(int n, int q, double Z[][ORC_NMAX], double eta) { /* Z_j *= 
   }
 }
 
+/* constant source terms: f <- f + s, one rounded addition per component after the network's own
+ * sums are complete (the Jacobian is unchanged: s does not depend on y).  src == NULL: f untouched. */
+static void add_source(int n, const double *src, double *f) {
+  if (!src) return;
+  for (int i = 0; i < n; i++) f[i] = f[i] + src[i];
+}
+
 /* one zone.  returns nst (>0) or a negative failure code; yout = last accepted state */
 static int burn_zone(const Net *nt, double rho, const double *y0, double dt, double rtol,
-                     double atol, const orc_opts *o, double *yout, uint64_t *cnt) {
+                     double atol, const orc_opts *o, const double *src, double *yout, uint64_t *cnt) {
   const int n = nt->n;
   const int L = (o && o->norm_lanes > 0) ? o->norm_lanes : 1;
   const int fixed = (o && o->fixed_q > 0);
@@ -399,9 +406,13 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
 
   for (int i = 0; i < n; i++) yout[i] = y0[i];
   if (!(rho > 0.0) || !isfinite(rho) || invalid_state(n, y0)) return -4;
+  if (src)
+    for (int i = 0; i < n; i++)
+      if (!isfinite(src[i])) return -4;
 
   /* Init */
   rates(nt, rho, y0, f, P);
+  add_source(nt->n, src, f);
   cnt[1]++, cnt[2]++;
   set_weights(n, y0, rtol, atol, w);
   double h;
@@ -461,6 +472,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
       for (int i = 0; i < n; i++) y[i] = Z[0][i];
       if (!invalid_state(n, y)) { /* B.3 */
         rates(nt, rho, y, f, P);
+        add_source(n, src, f);
         cnt[1]++, cnt[2]++;
         for (int i = 0; i < n; i++)
           for (int j = 0; j < n; j++) P[i * n + j] = fma(-gamma, P[i * n + j], (i == j) ? 1.0 : 0.0);
@@ -475,6 +487,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
               for (int i = 0; i < n; i++) y[i] = Z[0][i] + acor[i];
               if (invalid_state(n, y)) break;
               rates(nt, rho, y, f, NULL);
+              add_source(n, src, f);
               cnt[1]++;
             }
             for (int i = 0; i < n; i++) b[i] = fma(gamma, f[i], -fma(Z[1][i], rl1, acor[i]));
@@ -548,6 +561,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
         h = h * ETAMIN;
         for (int i = 0; i < n; i++) y[i] = Z[0][i];
         rates(nt, rho, y, f, NULL);
+              add_source(n, src, f);
         cnt[1]++;
         for (int i = 0; i < n; i++) Z[1][i] = h * f[i];
         nqwait = 10;
@@ -721,7 +735,13 @@ int orc_burn(const orc_net_desc *d, int64_t nz, const double *rho, const double 
       double y0[ORC_NMAX], yout[ORC_NMAX];
       for (int i = 0; i < N; i++) y0[SP(i)] = X[(int64_t)i * nz + z] / nt.aion[i];
       y0[TI] = T[z];
-      int code = burn_zone(&nt, rho[z], y0, dt, rtol, atol, opts, yout, cnt);
+      double srcv[ORC_NMAX];
+      const int has_src = opts && opts->src_T && opts->src_X;
+      if (has_src) {
+        for (int i = 0; i < N; i++) srcv[SP(i)] = opts->src_X[(int64_t)i * nz + z] / nt.aion[i];
+        srcv[TI] = opts->src_T[z];
+      }
+      int code = burn_zone(&nt, rho[z], y0, dt, rtol, atol, opts, has_src ? srcv : NULL, yout, cnt);
       if (code == -4) { /* invalid input: outputs = inputs */
         for (int i = 0; i < N; i++) X_out[(int64_t)i * nz + z] = X[(int64_t)i * nz + z];
         T_out[z] = T[z];

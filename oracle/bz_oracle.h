@@ -48,6 +48,11 @@ typedef struct {
   double fixed_h;      /* test hook: the fixed step                                       */
   const double *z_init;/* test hook: [(fixed_q+1)][n] initial Nordsieck array (scaled by fixed_h) */
   int32_t nthreads;    /* OpenMP threads over zones; <=0 = runtime default                */
+  /* constant per-zone source terms (SDC-style coupling): the system
+   * integrated is dy/dt = f(rho, y) + s with dT/dt += src_T[z] [K/s] and
+   * dY_i/dt += src_X[i][z] / A_i (src_X is a mass-fraction rate [1/s]).  NULL = no sources. */
+  const double *src_T; /* [nz] or NULL */
+  const double *src_X; /* [N][nz] or NULL (both or neither) */
 } orc_opts;
 
 /* counters[8] = {nst, nrhs, njac, nlu, nsolve, netf, ncfn, nfailzones} summed over zones */

@@ -21,7 +21,7 @@ class _Desc(C.Structure):
 
 class _Opts(C.Structure):
     _fields_ = [("norm_lanes", C.c_int32), ("fixed_q", C.c_int32), ("fixed_h", C.c_double),
-                ("z_init", _dp), ("nthreads", C.c_int32)]
+                ("z_init", _dp), ("nthreads", C.c_int32), ("src_T", _dp), ("src_X", _dp)]
 
 
 _lib = None
@@ -99,8 +99,11 @@ def max_threads() -> int:
     return int(_L().orc_max_threads())
 
 
-def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fixed_h=0.0, z_init=None):
-    """Integrate every zone over dt.  X: [nspec, nz].  Returns (T_out, X_out, nsteps, counters)."""
+def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fixed_h=0.0, z_init=None,
+         src_T=None, src_X=None):
+    """Integrate every zone over dt.  X: [nspec, nz].  Returns (T_out, X_out, nsteps, counters).
+    src_T [nz] (K/s) and src_X [nspec, nz] (mass-fraction rate, 1/s): optional constant source terms
+    (dy/dt = f + s, bz_oracle.h); give both or neither."""
     rho = np.ascontiguousarray(rho, dtype=np.float64)
     T = np.ascontiguousarray(T, dtype=np.float64)
     X = np.ascontiguousarray(X, dtype=np.float64)
@@ -114,8 +117,14 @@ def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fi
     zi = None
     if z_init is not None:
         zi = np.ascontiguousarray(z_init, dtype=np.float64)
+    assert (src_T is None) == (src_X is None)
+    sT = sX = None
+    if src_T is not None:
+        sT = np.ascontiguousarray(src_T, dtype=np.float64)
+        sX = np.ascontiguousarray(src_X, dtype=np.float64)
+        assert sT.shape == (nz,) and sX.shape == (d.nspec, nz)
     opts = _Opts(int(norm_lanes), int(fixed_q), float(fixed_h), _d(zi) if zi is not None else None,
-                 int(nthreads))
+                 int(nthreads), _d(sT) if sT is not None else None, _d(sX) if sX is not None else None)
     rc = _L().orc_burn(C.byref(d), nz, _d(rho), _d(T), _d(X), dt, rtol, atol, _d(T_out), _d(X_out),
                        _i(nsteps), C.byref(opts), cnt)
     if rc != 0:

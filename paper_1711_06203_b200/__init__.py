@@ -5,7 +5,7 @@ for sm_100a).  PyTorch is used for device memory and streams only.  There is no 
 without the built library or without a CUDA device every compute call raises.
 """
 from .binding import (  # noqa: F401
-    BurnError, Net, net_create, burn_zones, burn_zones_host, net_destroy, get_counters,
+    BurnError, Net, net_create, burn_zones, burn_zones_src, strang_step, burn_zones_host, net_destroy, get_counters,
     fp64_peak_probe, library_path, COUNTER_NAMES, EXPORTED_SYMBOLS,
 )
 from .sharding import shard_range, shard_workload  # noqa: F401

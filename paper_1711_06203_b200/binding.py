@@ -9,10 +9,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
-EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_host", "net_destroy", "bz_get_counters",
+EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_src", "burn_zones_host", "net_destroy", "bz_get_counters",
                     "bz_norm_lanes", "bz_select_kernel", "bz_kernel_name", "bz_last_cuda_error", "bz_fp64_peak_probe")
 _STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
-           -5: "CUDA runtime error", -6: "out of memory"}
+           -5: "CUDA runtime error", -6: "out of memory", -7: "unsupported by the forced kernel"}
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -33,7 +33,8 @@ class _Desc(C.Structure):
 
 
 def library_path() -> str:
-    return os.path.join(_HERE, "libburn.so")
+    """The in-tree build; BZ_LIBBURN names another build of the same library (kernel experiments)."""
+    return os.environ.get("BZ_LIBBURN") or os.path.join(_HERE, "libburn.so")
 
 
 _lib = None
@@ -59,6 +60,9 @@ def _L():
         lib.burn_zones.argtypes = sig
         lib.burn_zones_host.restype = C.c_int
         lib.burn_zones_host.argtypes = sig
+        lib.burn_zones_src.restype = C.c_int
+        lib.burn_zones_src.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp, C.c_double, C.c_double, C.c_double,
+                                       vp, vp, vp, vp]
         lib.bz_get_counters.restype = C.c_int
         lib.bz_get_counters.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
         lib.bz_norm_lanes.restype = C.c_int
@@ -176,6 +180,45 @@ def burn_zones(net: Net, rho, T, X, dt, rtol, atol, T_out=None, X_out=None, nste
     _check(_L().burn_zones(net._h, nz, p(rho), p(T), p(X), float(dt), float(rtol), float(atol),
                            p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones")
     return T_out, X_out, nsteps
+
+
+def burn_zones_src(net: Net, rho, T, X, src_T, src_X, dt, rtol, atol, T_out=None, X_out=None, nsteps=None,
+                   stream=None):
+    """burn_zones with constant per-zone source terms (include/burnzones.h: burn_zones_src):
+    dT/dt += src_T [nz] (K/s), dX_i/dt += src_X [nspec, nz] (1/s).  Device tensors like burn_zones."""
+    import torch
+    nz = rho.shape[0]
+    for name, t, shape in (("rho", rho, (nz,)), ("T", T, (nz,)), ("X", X, (net.nspec, nz)),
+                           ("src_T", src_T, (nz,)), ("src_X", src_X, (net.nspec, nz))):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
+            raise ValueError(f"{name} must be a contiguous float64 CUDA tensor of shape {shape}")
+    if T_out is None:
+        T_out = torch.empty_like(T)
+    if X_out is None:
+        X_out = torch.empty_like(X)
+    if nsteps is None:
+        nsteps = torch.empty(nz, dtype=torch.int32, device=rho.device)
+    for name, t, dt_, shape in (("T_out", T_out, torch.float64, (nz,)), ("X_out", X_out, torch.float64, (net.nspec, nz)),
+                                ("nsteps", nsteps, torch.int32, (nz,))):
+        if not (t.is_cuda and t.dtype == dt_ and t.is_contiguous() and tuple(t.shape) == shape):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {shape}")
+    p = lambda t: C.c_void_p(t.data_ptr())
+    _check(_L().burn_zones_src(net._h, nz, p(rho), p(T), p(X), p(src_T), p(src_X), float(dt), float(rtol),
+                               float(atol), p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones_src")
+    return T_out, X_out, nsteps
+
+
+def strang_step(net: Net, rho, T, X, dt, rtol, atol, update=None, stream=None):
+    """One Strang-split step of an operator-split code ("reactions are incorporated via operator
+    splitting", section 3.1): burn(dt/2), the caller's `update` (hydro/advection of
+    the state, any function (rho, T, X) -> (rho, T, X) of device tensors enqueued on the same
+    stream; None = identity), burn(dt/2).  Marshalling only: both halves are burn_zones calls.
+    Returns (rho, T, X, nsteps_first_half, nsteps_second_half); nothing is synchronised."""
+    T1, X1, ns1 = burn_zones(net, rho, T, X, 0.5 * dt, rtol, atol, stream=stream)
+    if update is not None:
+        rho, T1, X1 = update(rho, T1, X1)
+    T2, X2, ns2 = burn_zones(net, rho, T1, X1, 0.5 * dt, rtol, atol, stream=stream)
+    return rho, T2, X2, ns1, ns2
 
 
 def burn_zones_host(net: Net, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, stream=None):

@@ -44,6 +44,7 @@ struct BurnArgs {
   int *nsteps;
   unsigned long long *queue;     // work-queue head
   unsigned long long *counters;  // [8]
+  const double *src_T, *src_X;   // constant source terms (burn_zones_src), both nullptr = none
 };
 
 __device__ __forceinline__ double inv_small_int(int p) {  // 1.0/p, p = 1..7, correctly rounded

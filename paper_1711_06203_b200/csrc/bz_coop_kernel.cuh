@@ -17,6 +17,9 @@ struct Group {
   const int *rp, *sp_off, *sp_k, *cl_off, *cl_ks;
   // per-group scratch in shared memory
   double *ysh, *R, *dRdT, *dRdY, *M, *urow, *xs;
+  // constant source of my component (burn_zones_src); added to f after the network's own sums
+  bool has_src;
+  double src;
 
   __device__ __forceinline__ void sync() const { __syncwarp(gmask); }
 
@@ -177,6 +180,7 @@ struct Group {
       if (lig < n) M[lig] = fac * jt;  // row 0 = temperature equation
       sync();
     }
+    if (has_src) f = f + src;
     return f;
   }
 };

@@ -45,6 +45,8 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
     g.dRdY = g.dRdT + K;
     g.M = g.dRdY + 3 * K;
   }
+  g.has_src = (A.src_T != nullptr);
+  g.src = 0.0;
   const int lig = g.lig;
   const bool act = lig < n;      // lanes that own a component
   const double dt = A.dt, rtol = A.rtol, atol = A.atol;
@@ -84,7 +86,13 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
           xin = A.T[z];
         }
         const double y0 = (lig >= 1 && lig <= N) ? xin / ai : xin;
-        const bool bad = !(rho > 0.0) || !finite_(rho) || (act && !finite_(y0)) || (lig == 0 && !(y0 > 0.0));
+        if (g.has_src) {
+          g.src = 0.0;
+          if (lig >= 1 && lig <= N) g.src = A.src_X[(long long)(lig - 1) * A.nz + z] / ai;
+          else if (lig == 0) g.src = A.src_T[z];
+        }
+        const bool bad = !(rho > 0.0) || !finite_(rho) || (act && !finite_(y0)) || (lig == 0 && !(y0 > 0.0)) ||
+                         (g.has_src && !finite_(g.src));
         if (g.gany(bad)) {  // invalid input zone: outputs = inputs; stay in phase 0
           if (lig >= 1 && lig <= N) {
             A.X_out[(long long)(lig - 1) * A.nz + z] = xin;

@@ -45,7 +45,8 @@ struct QuadMem {
   static constexpr int SC_T = 26, SC_ETAMAX = 27, SC_HSAV = 28, SC_ZID = 29, SC_INT = 30, SC_N = 31;
   static constexpr int CNT_OFF = SC_OFF + SC_N;         // event counters of this quad: 8 x uint32 (lane 0 only)
   static constexpr int CN_NST = 0, CN_XRHS = 1, CN_INIT = 2, CN_LU = 3, CN_SOL = 4, CN_ETF = 5, CN_CFN = 6, CN_FAIL = 7;
-  static constexpr int RAW = CNT_OFF + 4;
+  static constexpr int SRC_OFF = CNT_OFF + 4;           // constant source terms s[NEQ] (burn_zones_src)
+  static constexpr int RAW = SRC_OFF + NEQ;
   static constexpr int SIZE = RAW + ((4 - (RAW % 32) + 32) % 32);  // == 4 (mod 32)
   double *base;
   __device__ __forceinline__ double &Z(int j, int i) const { return base[Z_OFF + j * NEQ + i]; }
@@ -57,6 +58,7 @@ struct QuadMem {
   __device__ __forceinline__ double &sc(int i) const { return base[SC_OFF + i]; }
   __device__ __forceinline__ long long &zid() const { return *reinterpret_cast<long long *>(base + SC_OFF + SC_ZID); }
   __device__ __forceinline__ int &isc(int i) const { return reinterpret_cast<int *>(base + SC_OFF + SC_INT)[i]; }  // 0: qS, 1: ntau
+  __device__ __forceinline__ double &src(int i) const { return base[SRC_OFF + i]; }
   __device__ __forceinline__ unsigned &cnt(int i) const { return reinterpret_cast<unsigned *>(base + CNT_OFF)[i]; }
 };
 

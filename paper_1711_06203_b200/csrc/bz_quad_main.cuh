@@ -35,6 +35,15 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   double *gP = qn.gscratch + gquad * (NEQ * NEQ + 2 * NEQ);  // general path: P, b, ipvt
   const double dt = A.dt, rtol = A.rtol, atol = A.atol, fac = qn.fac;
   const double inv_n = 1.0 / (double)NEQ;
+  const bool has_src = (A.src_T != nullptr);  // burn_zones_src: f <- f + s after every rate evaluation
+  // (each lane adds the sources of its own components; they sit in the zone's shared memory)
+#define BZQ_ADD_SRC(fv)                                         \
+  do {                                                          \
+    if (has_src) {                                              \
+      _Pragma("unroll") for (int s_ = 0; s_ < S; s_++)          \
+        if (BZQ_OK(s_)) fv[s_] = fv[s_] + m.src(BZQ_I(s_));     \
+    }                                                           \
+  } while (0)
   // event counters live in the quad's shared memory (lane 0 counts): registers are the scarce
   // resource of this kernel.  nrhs = nlu + ninit + xrhs and njac = nlu + ninit are derived at the end.
 #define BZQ_COUNT(k) do { if (c == 0) m.cnt(Mem::k) += 1u; } while (0)
@@ -125,6 +134,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             y[s] = xin[s] / aion[i - 1];
             bad |= !finite_(y[s]);
           }
+          if (has_src && i < NEQ) {
+            const double sv = (i == 0) ? A.src_T[z] : A.src_X[(long long)(i - 1) * A.nz + z] / aion[i - 1];
+            m.src(i) = sv;  // own component only: no intra-quad hazard
+            bad |= !finite_(sv);
+          }
         }
         if (qany(bad)) {  // invalid input zone: outputs = inputs, stay in phase 0
 #pragma unroll
@@ -149,6 +163,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             }
           __syncwarp(gmask);
           Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, f, lu.a);
+          BZQ_ADD_SRC(f);
           BZQ_COUNT(CN_INIT);
           // exact second derivative y'' = J f for the first step size
           __syncwarp(gmask);
@@ -195,6 +210,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
 #undef BZQ_SEG_SYNC
   // ---- counters (lane 0 of each quad holds the zone's counts) ------------------------------------
 #undef BZQ_COUNT
+#undef BZQ_ADD_SRC
 #undef BZQ_T
 #undef BZQ_ETAMAX
 #undef BZQ_HSAV

@@ -379,6 +379,12 @@ int bz_select_kernel(bz_net *h, int kind) {
 int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
                double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
                void *cuda_stream) {
+  return burn_zones_src(h, nz, rho, T, X, nullptr, nullptr, dt, rtol, atol, T_out, X_out, nsteps, cuda_stream);
+}
+
+int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+                   const double *src_T, const double *src_X, double dt, double rtol, double atol,
+                   double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream) {
   if (!h) return BZ_ERR_NULL;
   if (nz < 0) return BZ_ERR_SIZE;
   if (!(dt > 0.0) || !(rtol > 0.0) || !(atol >= 0.0) || !std::isfinite(dt) || !std::isfinite(rtol) ||
@@ -386,9 +392,12 @@ int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, 
     return BZ_ERR_SCALAR;
   if (nz == 0) return BZ_OK;
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
+  if (src_T && !use_quad(h) && use_tpz(h)) return BZ_ERR_UNSUPPORTED;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   BZ_CUDA(cudaMemsetAsync(h->d_scratch, 0, 16 * sizeof(unsigned long long), st));
   bz::BurnArgs a;
+  a.src_T = src_T; a.src_X = src_X;
   a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
