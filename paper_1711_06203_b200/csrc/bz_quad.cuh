@@ -100,11 +100,15 @@ struct QuadLU {
 
   // no-interchange factorisation.  returns bit 0: an interchange may be needed (results invalid,
   // redo on the general path), bit 1: zero / NaN pivot.  Quad-uniform result.
-  // Interchange test: LINPACK swaps iff some |a_ik| > |a_kk| below the diagonal, i.e. iff the exact
-  // quotient exceeds 1 in magnitude.  The computed multiplier l = RN(a_ik * RN(1/a_kk)) is within
-  // 2 ulp of that quotient, so |l| < 1 - 2^-21 (high word below 0x3FEFFFFF) proves that no swap is
-  // needed; anything else (near-ties, exact ties, NaN) takes the general path, which pivots exactly.
-  // Cost: one AND and one unsigned max per multiplier instead of a compare-and-select chain.
+  // Interchange test: LINPACK swaps iff some |a_ik| > |a_kk| below the diagonal.  Then
+  // |a_ik| >= |a_kk| (1 + 2^-52), and with inv = RN(1/a_kk) = (1 + e)/a_kk, |e| <= 2^-53, the exact
+  // product |a_ik * inv| >= (1 + 2^-52)(1 - 2^-53) > 1, so the computed multiplier
+  // l = RN(a_ik * inv) has |l| >= 1 (rounding is monotone).  Hence |l| < 1 -- high word below
+  // 0x3FF00000, one AND and one unsigned max per multiplier -- PROVES that dgefa would not swap.
+  // |l| >= 1 without a swap needs |a_ik| within one ulp of |a_kk| (exact ties included); those and
+  // NaN multipliers take the general path, which pivots exactly.  (A bound of 1 - 2^-21 was
+  // tried first: stiff steps approach |l| -> 1 from below and sent the hot zones of config 4 to the
+  // general path often enough to cost 18 % of that config.)
   // b: right-hand side of the first solve; its forward elimination (dgesl, k ascending) rides along:
   // the pivot row's b_k is published with the row, so the first solve needs only back_solve().
   template <class Mem>
@@ -147,7 +151,7 @@ struct QuadLU {
         }
       }
     }
-    const unsigned f = (lmax >= 0x3FEFFFFFu ? 1u : 0u) | (bad ? 2u : 0u);
+    const unsigned f = (lmax >= 0x3FF00000u ? 1u : 0u) | (bad ? 2u : 0u);
     // make the flags quad-uniform
     unsigned r = f;
     r |= __shfl_xor_sync(gmask, r, 1, 4);
