@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
     return sqrt(p * inv_n);
   };
 
-  int phase = 0;  // 0 need a zone, 1 stepping, 2 queue empty
+  int phase = 0;  // 0 need a zone, 1 stepping, 2 queue empty, 3 zone loaded: initial rates pending
   double rho = 0.0, h = 0.0;
   int q = 1, nqwait = 2, nst = 0, ncf = 0, nef = 0;
   // t, etamax, h_S, q_S, ntau and the zone index live in the zone's shared memory (bz_quad.cuh)
@@ -108,6 +108,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   QuadLU<NEQ> lu;
 
   for (unsigned trip = 0;; trip++) {
+    // zone starts: few per warp and trip while zones take hundreds of steps (config 3), all eight
+    // quads every trip where zones take one step (config 4).  Every thread votes here.
+    const bool bulk = __popc(__ballot_sync(0xffffffffu, phase == 0)) >= 8;  // two quads or more
     if (phase == 0) {
       // ---- a2 + a1: next zone, load, validate, initialise ------------------------------------------
       long long z = 0;
@@ -152,50 +155,73 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
           }
           BZQ_COUNT(CN_FAIL);
         } else {
-          double f[S], v[S];
-          __syncwarp(gmask);
+          if (bulk) {
+            // several quads of the warp start a zone in this trip: initialise here and now, so that a
+            // one-step zone (the cold regions of config 4) costs one trip
+            double f[S], v[S];
+            __syncwarp(gmask);
 #pragma unroll
-          for (int s = 0; s < S; s++)
-            if (BZQ_OK(s)) {
-              m.ysh()[BZQ_I(s)] = y[s];
-              m.W(BZQ_I(s)) = 1.0 / fma_(rtol, fabs(y[s]), atol);
-              m.Z(0, BZQ_I(s)) = y[s];
+            for (int s = 0; s < S; s++)
+              if (BZQ_OK(s)) {
+                m.ysh()[BZQ_I(s)] = y[s];
+                m.W(BZQ_I(s)) = 1.0 / fma_(rtol, fabs(y[s]), atol);
+                m.Z(0, BZQ_I(s)) = y[s];
+              }
+            __syncwarp(gmask);
+            Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, 0.0, f, lu.a);
+            BZQ_ADD_SRC(f);
+            BZQ_COUNT(CN_INIT);
+            // exact second derivative y'' = J f for the first step size
+            __syncwarp(gmask);
+#pragma unroll
+            for (int s = 0; s < S; s++)
+              if (BZQ_OK(s)) m.ysh()[BZQ_I(s)] = f[s];
+            __syncwarp(gmask);
+#pragma unroll
+            for (int s = 0; s < S; s++) {
+              double acc = 0.0;
+#pragma unroll
+              for (int j = 0; j < NEQ; j++) acc = fma_(lu.a[s][j], m.ysh()[j], acc);
+              v[s] = acc;
             }
-          __syncwarp(gmask);
-          Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, f, lu.a);
-          BZQ_ADD_SRC(f);
-          BZQ_COUNT(CN_INIT);
-          // exact second derivative y'' = J f for the first step size
-          __syncwarp(gmask);
+            const double d2 = wrms(v);
+            h = dt;
+            if (d2 > 0.0) {
+              const double hh = 0.5 * sqrt(2.0 / d2);
+              if (hh < dt) h = hh;
+            }
 #pragma unroll
-          for (int s = 0; s < S; s++)
-            if (BZQ_OK(s)) m.ysh()[BZQ_I(s)] = f[s];
-          __syncwarp(gmask);
+            for (int s = 0; s < S; s++)
+              if (BZQ_OK(s)) m.Z(1, BZQ_I(s)) = h * f[s];
+            q = 1, nqwait = 2, nst = 0;
+            BZQ_QS = 0, BZQ_NTAU = 0;
+            BZQ_T = 0.0, BZQ_ETAMAX = ETAMX1, BZQ_HSAV = 0.0;
+            if (c == 0) {
 #pragma unroll
-          for (int s = 0; s < S; s++) {
-            double acc = 0.0;
+              for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;
+            }
+            newstep = true;
+            phase = 1;
+          } else {
+            // publish y0; the first rate evaluation (f0, J0) rides along with the warp-uniform attempt
+            // of this trip (phase 3, bz_quad_attempt.inc), stepping starts with the next trip
+            __syncwarp(gmask);
 #pragma unroll
-            for (int j = 0; j < NEQ; j++) acc = fma_(lu.a[s][j], m.ysh()[j], acc);
-            v[s] = acc;
+            for (int s = 0; s < S; s++)
+              if (BZQ_OK(s)) {
+                m.ysh()[BZQ_I(s)] = y[s];
+                m.W(BZQ_I(s)) = 1.0 / fma_(rtol, fabs(y[s]), atol);
+                m.Z(0, BZQ_I(s)) = y[s];
+              }
+            q = 1, nqwait = 2, nst = 0;
+            BZQ_QS = 0, BZQ_NTAU = 0;
+            BZQ_T = 0.0, BZQ_ETAMAX = ETAMX1, BZQ_HSAV = 0.0;
+            if (c == 0) {
+#pragma unroll
+              for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;
+            }
+            phase = 3;
           }
-          const double d2 = wrms(v);
-          h = dt;
-          if (d2 > 0.0) {
-            const double hh = 0.5 * sqrt(2.0 / d2);
-            if (hh < dt) h = hh;
-          }
-#pragma unroll
-          for (int s = 0; s < S; s++)
-            if (BZQ_OK(s)) m.Z(1, BZQ_I(s)) = h * f[s];
-          q = 1, nqwait = 2, nst = 0;
-          BZQ_QS = 0, BZQ_NTAU = 0;
-          BZQ_T = 0.0, BZQ_ETAMAX = ETAMX1, BZQ_HSAV = 0.0;
-          if (c == 0) {
-#pragma unroll
-            for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;
-          }
-          newstep = true;
-          phase = 1;
         }
       }
     }
