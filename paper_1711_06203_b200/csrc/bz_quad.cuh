@@ -88,6 +88,37 @@ __device__ __forceinline__ double nord_shift(const Mem &m, int i, int q) {
   }
 }
 
+// One component's column of the Nordsieck array (z[j * STRIDE], j = 0..Q): retract the prediction
+// (same loop order as the predictor, C.2-B.7) and rescale by eta^j, for a compile-time order.
+template <int Q, int STRIDE>
+__device__ __forceinline__ void nord_retract_rescale_q(double *z, double eta) {
+  double zc[Q + 1];
+#pragma unroll
+  for (int j = 0; j <= Q; j++) zc[j] = z[j * STRIDE];
+#pragma unroll
+  for (int k = 1; k <= Q; k++)
+#pragma unroll
+    for (int j = Q; j >= k; j--) zc[j - 1] = zc[j - 1] - zc[j];
+  double r = eta;
+#pragma unroll
+  for (int j = 1; j <= Q; j++) {
+    zc[j] = zc[j] * r;
+    r = r * eta;
+  }
+#pragma unroll
+  for (int j = 0; j <= Q; j++) z[j * STRIDE] = zc[j];
+}
+template <int STRIDE>
+__device__ __forceinline__ void nord_retract_rescale(double *z, int q, double eta) {
+  switch (q) {
+    case 1: nord_retract_rescale_q<1, STRIDE>(z, eta); break;
+    case 2: nord_retract_rescale_q<2, STRIDE>(z, eta); break;
+    case 3: nord_retract_rescale_q<3, STRIDE>(z, eta); break;
+    case 4: nord_retract_rescale_q<4, STRIDE>(z, eta); break;
+    default: nord_retract_rescale_q<5, STRIDE>(z, eta); break;
+  }
+}
+
 template <int NEQ>
 struct QuadLU {
   static constexpr int S = (NEQ + 3) / 4;
