@@ -119,6 +119,27 @@ __device__ __forceinline__ void nord_retract_rescale(double *z, int q, double et
   }
 }
 
+// Z_j *= eta^j, j = 1..Q, powers by repeated multiplication (nord_rescale)
+template <int Q, int STRIDE>
+__device__ __forceinline__ void nord_rescale_only_q(double *z, double eta) {
+  double r = eta;
+#pragma unroll
+  for (int j = 1; j <= Q; j++) {
+    z[j * STRIDE] = z[j * STRIDE] * r;
+    r = r * eta;
+  }
+}
+template <int STRIDE>
+__device__ __forceinline__ void nord_rescale_only(double *z, int q, double eta) {
+  switch (q) {
+    case 1: nord_rescale_only_q<1, STRIDE>(z, eta); break;
+    case 2: nord_rescale_only_q<2, STRIDE>(z, eta); break;
+    case 3: nord_rescale_only_q<3, STRIDE>(z, eta); break;
+    case 4: nord_rescale_only_q<4, STRIDE>(z, eta); break;
+    default: nord_rescale_only_q<5, STRIDE>(z, eta); break;
+  }
+}
+
 template <int NEQ>
 struct QuadLU {
   static constexpr int S = (NEQ + 3) / 4;
