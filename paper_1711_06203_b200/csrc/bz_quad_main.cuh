@@ -22,15 +22,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   const int c = threadIdx.x & 3;
   const unsigned gmask = 0xfu << ((threadIdx.x & 31) & ~3);
   Mem m;
-#ifdef BZ_QUAD_OPAQUE_BASE
-  {
-    int zoff = ((4 * K + N + 1) & ~1) + (threadIdx.x >> 2) * Mem::SIZE;
-    asm volatile("" : "+r"(zoff));  // opaque: kept in a register instead of being recomputed from %tid at every use
-    m.base = smem + zoff;
-  }
-#else
   m.base = smem + ((4 * K + N + 1) & ~1) + (threadIdx.x >> 2) * Mem::SIZE;
-#endif
   const long long gquad = (long long)blockIdx.x * (QUAD_THREADS / 4) + (threadIdx.x >> 2);
   double *gP = qn.gscratch + gquad * (NEQ * NEQ + 2 * NEQ);  // general path: P, b, ipvt
   const double dt = A.dt, rtol = A.rtol, atol = A.atol, fac = qn.fac;
