@@ -11,10 +11,11 @@
 // The Nordsieck array, weights and the saved vector live in shared memory per zone.
 // LU (a5): the unknowns are ordered temperature-first, so partial pivoting
 // keeps the natural order almost always: step k's pivot row is the static (lane k%4, slot k/4);
-// it is published through shared memory, every lane verifies |a_ik| <= |a_kk| on its own rows
-// (exact), computes its own multipliers and updates its own rows.  A zone that does need an
-// interchange redoes the factorisation on the general path (lane 0 of the quad, LINPACK dgefa on
-// a global-memory scratch copy), bit-identical to the oracle either way.
+// it is published through shared memory, every lane computes its own multipliers, updates its own
+// rows and keeps the largest |multiplier|: below 1 it proves that dgefa would not have swapped
+// (QuadLU::factor).  A zone that may need an interchange redoes the factorisation on the general
+// path (lane 0 of the quad, LINPACK dgefa on a global-memory scratch copy), bit-identical to the
+// oracle either way.
 #pragma once
 #include <cstdint>
 #include "bz_coop.cuh"      // constants, BurnArgs, eta_of, factorial_, inv_small_int
