@@ -13,5 +13,7 @@ from .configs import (  # noqa: F401
     network_for_config,
     make_workload,
     first_order_decay_network,
+    aprox13_like_network,
+    make_aprox13_like_workload,
     sha256_of,
 )

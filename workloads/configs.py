@@ -189,6 +189,54 @@ def network_for_config(config: int) -> Network:
     raise ValueError(f"unknown config {config}")
 
 
+def aprox13_like_network(seed: int = 6) -> Network:
+    """A second 13-isotope workload in the style of the networks the paper's Fig. 5 ran
+    (SURVEY.md 8(f)-4): the alpha chain of config 3 with ALPHA-EMITTING heavy-ion
+    channels (C12+C12 -> Ne20 + a, C12+O16 -> Mg24 + a, O16+O16 -> Si28 + a) and the eleven REVERSE
+    (photodisintegration) links X_{m+1} -> X_m + a as first-order reactions.  The rate data are
+    synthetic (the real fits are not available and are not reproduced): forward coefficients as in
+    config 2 from ``default_rng(seed)``; reverse links A = 10^(10 u), n in [-1,1], B in [60,120]
+    (they switch on at high temperature) and Q = -Q of the matching capture.  26 reactions; runs on
+    the generic cooperative kernel (no generated code for this topology: its LU needs interchanges)."""
+    rng = np.random.default_rng(seed)
+    sp = ["He4", "C12", "O16", "Ne20", "Mg24", "Si28", "S32", "Ar36", "Ca40",
+          "Ti44", "Cr48", "Fe52", "Ni56"]
+    aion = np.empty(13)
+    aion[0] = 4.0
+    aion[1:] = 12.0 + 4.0 * np.arange(12)
+    reactants = [[0, 0, 0]]
+    stoich = [[(0, -3.0), (1, +1.0)]]
+    for x in range(1, 12):         # eleven (a,g) captures
+        reactants.append([x, 0])
+        stoich.append([(x, -1.0), (0, -1.0), (x + 1, +1.0)])
+    reactants.append([1, 1]); stoich.append([(1, -2.0), (3, +1.0), (0, +1.0)])             # C12+C12 -> Ne20 + a
+    reactants.append([1, 2]); stoich.append([(1, -1.0), (2, -1.0), (4, +1.0), (0, +1.0)])  # C12+O16 -> Mg24 + a
+    reactants.append([2, 2]); stoich.append([(2, -2.0), (5, +1.0), (0, +1.0)])             # O16+O16 -> Si28 + a
+    A, n, B, Q = _coeffs(rng, 15)
+    uA, un, uB = rng.random(11), rng.random(11), rng.random(11)
+    for x in range(1, 12):         # reverse links X_{x+1} -> X_x + a
+        reactants.append([x + 1])
+        stoich.append([(x + 1, -1.0), (x, +1.0), (0, +1.0)])
+    A = np.concatenate([A, 10.0 ** (10.0 * uA)])
+    n = np.concatenate([n, -1.0 + 2.0 * un])
+    B = np.concatenate([B, 60.0 + 60.0 * uB])
+    Q = np.concatenate([Q, -Q[1:12]])
+    reactant, sid, sdy = _pack(26, reactants, stoich)
+    return Network("aprox13like", sp, aion, reactant, sid, sdy, A, n, B, Q)
+
+
+def make_aprox13_like_workload(nz: int, seed: int = 6, dt: float = 1e-6) -> Workload:
+    """``nz`` zones for ``aprox13_like_network``: rho log-uniform [1e6, 1e8], T uniform [1e9, 4e9]
+    (hot enough for the reverse links to matter), X = Dirichlet(1) over He4/C12/O16/Si28/Ni56."""
+    net = aprox13_like_network(seed)
+    rng = np.random.default_rng(seed + 1000)
+    u_rho, u_T = rng.random(nz), rng.random(nz)
+    g = -np.log1p(-rng.random((5, nz)))
+    X = np.zeros((13, nz))
+    X[[0, 1, 2, 5, 12]] = g / g.sum(axis=0)
+    return Workload(6, net, 10.0 ** (6.0 + 2.0 * u_rho), 1e9 + 3e9 * u_T, X, dt, nz_full=nz)
+
+
 def first_order_decay_network(lam: float, q_mev: float = 0.0) -> Network:
     """i -> k, one first-order reaction with a temperature-independent rate
     (n = 0, B = 0): the closed-form pin named by north_star."""
