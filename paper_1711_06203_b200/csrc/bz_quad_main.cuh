@@ -47,13 +47,6 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   // component index of my slot s and its validity
 #define BZQ_I(s) (4 * (s) + c)
 #define BZQ_OK(s) (4 * (s) + c < NEQ)
-  // optional barriers between the segments of an attempt (measured slower than one barrier per
-  // trip: they serialise the pipes; kept as a switch)
-#ifdef BZ_QUAD_SEGMENT_BARRIERS
-#define BZQ_SEG_SYNC() __syncthreads()
-#else
-#define BZQ_SEG_SYNC() ((void)0)
-#endif
 
   auto qsum = [&](double v) {  // quad butterfly, strides 2 then 1 (norm_lanes = 4)
     v = v + __shfl_xor_sync(gmask, v, 2, 4);
@@ -217,15 +210,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
         }
       }
     }
-#ifdef BZ_QUAD_BARRIER_EVERY2
-    if ((trip & 1u) == 0u)
-#endif
-      if (__syncthreads_and(phase == 2)) break;
+    if (__syncthreads_and(phase == 2)) break;
 #include "bz_quad_attempt.inc"
   }
 #undef BZQ_I
 #undef BZQ_OK
-#undef BZQ_SEG_SYNC
   // ---- counters (lane 0 of each quad holds the zone's counts) ------------------------------------
 #undef BZQ_COUNT
 #undef BZQ_ADD_SRC
