@@ -139,14 +139,23 @@ struct Group {
       }
     }
     sync();
-    double f = 0.0;
+    double f = 0.0, jt0 = 0.0;
     const int sp = lig - 1;  // my species (lanes 1..N); lane 0 owns T
     if (lig >= 1 && lig <= N) {
       const int e = sp_off[sp + 1];
       for (int t = sp_off[sp]; t < e; t++) f = fma_(sp_dy[t], R[sp_k[t]], f);
     } else if (lig == 0) {
+      // the temperature lane sums over ALL reactions: its two K-term chains (energy rate and
+      // d/dT of it) share one loop, so the single active lane has two independent FMAs in flight
       double s = 0.0;
-      for (int k = 0; k < K; k++) s = fma_(Q[k], R[k], s);
+      if (WITH_J) {
+        for (int k = 0; k < K; k++) {
+          s = fma_(Q[k], R[k], s);
+          jt0 = fma_(Q[k], dRdT[k], jt0);
+        }
+      } else {
+        for (int k = 0; k < K; k++) s = fma_(Q[k], R[k], s);
+      }
       f = fac * s;
     }
     if (WITH_J) {
@@ -174,7 +183,7 @@ struct Group {
           jt = fma_(Q[ks & 0xffff], dRdY[3 * (ks & 0xffff) + (ks >> 16)], jt);
         }
       } else if (lig == 0) {
-        for (int k = 0; k < K; k++) jt = fma_(Q[k], dRdT[k], jt);
+        jt = jt0;  // summed alongside f above (same k-ascending fma chain)
       }
       sync();  // rows of the species are complete before the T row is written
       if (lig < n) M[lig] = fac * jt;  // row 0 = temperature equation
