@@ -5,4 +5,5 @@ import this package.  It never imports paper_1711_06203_b200 and vice versa.
 """
 from .oracle import (  # noqa: F401
     burn, rates, oexp, olog, lu_factor, lu_solve, bdf_coeffs, wrms, max_threads, interchanges, event_counts, COUNTER_NAMES,
+    build_d, TRACE_FIELDS,
 )

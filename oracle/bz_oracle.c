@@ -148,8 +148,11 @@ static int net_init(Net *nt, const orc_net_desc *d) {
  *   R_k = ((lambda_k rho^(m-1)) invsym_k) * Y_r0 * Y_r1 * Y_r2
  *   dR_k/dY_j = pref_k * sum_{positions a: r[a]=j} prod_{b != a} Y_r[b]   (never R/Y)
  *   dR_k/dT   = R_k (n_k + B_k t13/3) / T
- * All Y above are Y+ = max(Y, 0): abundances that the integrator lets dip below zero (by
- * ~atol) do not feed the rate products, which would otherwise be unstable (reading s19).
+ * Negative abundances (the integrator lets trace species dip to ~ -atol), reading s19: the ODD,
+ * MONOTONE EXTENSION.  Products are formed from |Y|; if ANY reactant of reaction k is negative the
+ * rate is R_k = -pref_k prod|Y_r| (else +pref_k prod Y_r); dR_k/dY_j = pref_k d(prod|Y|)/d|Y_j|,
+ * negated when some reactant is negative UNLESS species j itself is (then d|Y_j|/dY_j = -1 cancels
+ * the sign of the rate).  Equal to the raw product law whenever at most one factor is negative.
  * Accumulation order: reactions k ascending; per reaction the stoichiometry entries in table
  * order; the temperature row accumulates sum_k Q_k (.) and is scaled by fac at the end. */
 /* Internal ordering of the unknowns (reading s25): y = (T, Y_0, ..., Y_{N-1}),
@@ -349,6 +352,8 @@ static void build_d(int cnt, const double *xi, double *d) {
   }
 }
 
+void orc_build_d(int cnt, const double *xi, double *d) { build_d(cnt, xi, d); }
+
 /* eta = 1 / ((bias*E)^(1/p) + ADDON), the root through the own exp/log */
 static double eta_of(double E, double bias, int p) {
   double v = bias * E;
@@ -391,18 +396,47 @@ static void add_source(int n, const double *src, double *f) {
   for (int i = 0; i < n; i++) f[i] = f[i] + src[i];
 }
 
+/* test hook (orc_opts.trace): copy one event record out; no arithmetic of the method here */
+typedef struct {
+  double *buf;
+  int cap, n_unk, count;
+} Trace;
+static void trace_put(Trace *tr, const double head[ORC_TRACE_HEAD], double Zacc[][ORC_NMAX],
+                      double Zend[][ORC_NMAX]) {
+  if (!tr || !tr->buf) return;
+  const int n = tr->n_unk;
+  if (tr->count < tr->cap) {
+    double *r = tr->buf + (size_t)tr->count * (ORC_TRACE_HEAD + 12 * n);
+    for (int i = 0; i < ORC_TRACE_HEAD; i++) r[i] = head[i];
+    for (int j = 0; j <= QMAX; j++)
+      for (int i = 0; i < n; i++) { /* API order: T last */
+        const int e = (i == TI) ? n - 1 : i - 1;
+        r[ORC_TRACE_HEAD + j * n + e] = Zacc ? Zacc[j][i] : 0.0;
+        r[ORC_TRACE_HEAD + (6 + j) * n + e] = Zend[j][i];
+      }
+  }
+  tr->count++;
+}
+
 /* one zone.  returns nst (>0) or a negative failure code; yout = last accepted state */
 static int burn_zone(const Net *nt, double rho, const double *y0, double dt, double rtol,
-                     double atol, const orc_opts *o, const double *src, double *yout, uint64_t *cnt) {
+                     double atol, const orc_opts *o, const double *src, double *yout, uint64_t *cnt,
+                     Trace *tr) {
   const int n = nt->n;
   const int L = (o && o->norm_lanes > 0) ? o->norm_lanes : 1;
   const int fixed = (o && o->fixed_q > 0);
+  const int mxstep = (o && o->mxstep > 0) ? o->mxstep : MXSTEP;
+  const int mxnef = (o && o->mxnef > 0) ? o->mxnef : MXNEF;
+  const int mxncf = (o && o->mxncf > 0) ? o->mxncf : MXNCF;
   double Z[QMAX + 2][ORC_NMAX], S[ORC_NMAX], w[ORC_NMAX], acor[ORC_NMAX], y[ORC_NMAX];
   double f[ORC_NMAX], b[ORC_NMAX], vtmp[ORC_NMAX];
   double P[ORC_NMAX * ORC_NMAX], inv[ORC_NMAX];
   int32_t ipvt[ORC_NMAX];
   double tau[8] = {0}, l[8], hs[8], rxi[8], xi[8], d[8];
   int ntau = 0;
+  double Zacc[QMAX + 2][ORC_NMAX], thead[ORC_TRACE_HEAD]; /* trace hook only */
+  for (int j = 0; j < QMAX + 2; j++)
+    for (int i = 0; i < ORC_NMAX; i++) Z[j][i] = 0.0, Zacc[j][i] = 0.0;
 
   for (int i = 0; i < n; i++) yout[i] = y0[i];
   if (!(rho > 0.0) || !isfinite(rho) || invalid_state(n, y0)) return -4;
@@ -516,7 +550,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
         ncf++, cnt[6]++;
         etamax = 1.0;
         last = 0;
-        if (ncf > MXNCF) {
+        if (ncf > mxncf) {
           for (int i = 0; i < n; i++) yout[i] = Z[0][i];
           return -1;
         }
@@ -526,12 +560,13 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
       }
       /* B.5 error test */
       dsm = orc_wrms(n, acor, w, L) / cerr;
-      if (fixed || dsm <= 1.0) break; /* accept */
+      const int injected = (o && o->inject_nef > 0 && nst + 1 == o->inject_step && nef < o->inject_nef);
+      if (fixed || (dsm <= 1.0 && !injected)) break; /* accept (test hook: see orc_opts.inject_step) */
       retract(n, q, Z);
       nef++, cnt[5]++;
       etamax = 1.0;
       last = 0;
-      if (nef == MXNEF) {
+      if (nef == mxnef) {
         for (int i = 0; i < n; i++) yout[i] = Z[0][i];
         return -2;
       }
@@ -554,7 +589,20 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
           for (int i = 0; i < n; i++) Z[j][i] = fma(-d[j], Z[q][i], Z[j][i]);
         q = q - 1;
         nqwait = q + 1;
+        double Zpre[QMAX + 2][ORC_NMAX]; /* trace hook only: the lowered array on the scale h_used */
+        if (tr)
+          for (int j = 0; j <= QMAX; j++)
+            for (int i = 0; i < n; i++) Zpre[j][i] = (j <= q) ? Z[j][i] : 0.0;
         rescale(n, q, Z, ETAMIN);
+        if (tr) {
+          double hd[ORC_TRACE_HEAD] = {1.0, t, h, (double)(q + 1), dsm, 0, 0, 0, 0, 0, -1.0, ETAMIN,
+                                       h * ETAMIN, (double)q, (double)nef, (double)ncf};
+          for (int j = q + 1; j <= QMAX; j++)
+            for (int i = 0; i < n; i++) Zacc[j][i] = 0.0;
+          for (int j = 0; j <= q; j++)
+            for (int i = 0; i < n; i++) Zacc[j][i] = Z[j][i];
+          trace_put(tr, hd, Zpre, Zacc);
+        }
         h = h * ETAMIN;
       } else {
         ORC_EVENT(2);
@@ -565,6 +613,15 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
         cnt[1]++;
         for (int i = 0; i < n; i++) Z[1][i] = h * f[i];
         nqwait = 10;
+        if (tr) {
+          double hd[ORC_TRACE_HEAD] = {2.0, t, h / ETAMIN, 1.0, dsm, 0, 0, 0, 0, 0, 0.0, ETAMIN,
+                                       h, 1.0, (double)nef, (double)ncf};
+          for (int j = 2; j <= QMAX; j++)
+            for (int i = 0; i < n; i++) Zacc[j][i] = 0.0;
+          for (int j = 0; j <= 1; j++)
+            for (int i = 0; i < n; i++) Zacc[j][i] = Z[j][i];
+          trace_put(tr, hd, NULL, Zacc);
+        }
       }
     }
     /* C. accept */
@@ -574,15 +631,23 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
     nst++;
     cnt[0]++;
     set_weights(n, Z[0], rtol, atol, w);
+    if (tr) {
+      for (int j = 0; j <= QMAX; j++)
+        for (int i = 0; i < n; i++) Zacc[j][i] = (j <= q) ? Z[j][i] : 0.0;
+      const double hd[ORC_TRACE_HEAD] = {0.0, t, h, (double)q, dsm, 0, 0, 0, 0, 0, 0.0, 1.0,
+                                         h, (double)q, (double)nef, (double)ncf};
+      for (int i = 0; i < ORC_TRACE_HEAD; i++) thead[i] = hd[i];
+      if (last || nst == mxstep) trace_put(tr, thead, Zacc, Zacc);
+    }
     if (last) break;
-    if (nst == MXSTEP) {
+    if (nst == mxstep) {
       for (int i = 0; i < n; i++) yout[i] = Z[0][i];
       return -3;
     }
     /* D. select next step and order */
     double eta = 1.0;
     int action = 0; /* -1 lower, 0 keep, +1 raise */
-    if (!fixed) {
+    if (!fixed || tr) { /* (fixed-q hook: evaluated for the trace only, never applied -- see below) */
       nqwait--;
       if (etamax == 1.0) {
         if (nqwait < 2) nqwait = 2;
@@ -601,6 +666,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
             }
             double Em = orc_wrms(n, Z[q], w, L) / (pm * sm);
             etaqm1 = eta_of(Em, BIAS1, q);
+            if (tr) thead[8] = Em;
           }
           if (q < QMAX && qS == q && ntau >= q) {
             double rq1 = h / (hs[q] + tau[q]); /* 1/xi_{q+1} */
@@ -617,7 +683,9 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
             for (int i = 0; i < n; i++) vtmp[i] = fma(cq, acor[i], -(rs * S[i]));
             double Ep = orc_wrms(n, vtmp, w, L) / ((pp * sp) * FACT[q + 2]);
             etaqp1 = eta_of(Ep, BIAS3, q + 2);
+            if (tr) thead[9] = Ep;
           }
+          if (tr) thead[5] = etaq, thead[6] = etaqm1, thead[7] = etaqp1;
           if (etaq >= etaqp1) {
             if (etaq >= etaqm1) {
               eta = etaq;
@@ -647,6 +715,10 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
         hS = h;
         qS = q;
       }
+      if (fixed) { /* fixed-q, fixed-h hook: the selection above is reported, not applied */
+        eta = 1.0;
+        action = 0;
+      }
     }
     /* E. apply (xi_i = hs[i]/h of B.1) */
     if (action == -1) {
@@ -675,6 +747,13 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
     if (eta != 1.0) {
       rescale(n, q, Z, eta);
       h = h * eta;
+    }
+    if (tr) {
+      thead[10] = (double)action, thead[11] = eta, thead[12] = h, thead[13] = (double)q;
+      double Zend[QMAX + 2][ORC_NMAX];
+      for (int j = 0; j <= QMAX; j++)
+        for (int i = 0; i < n; i++) Zend[j][i] = (j <= q) ? Z[j][i] : 0.0;
+      trace_put(tr, thead, Zacc, Zend);
     }
   }
   for (int i = 0; i < n; i++) yout[i] = Z[0][i];
@@ -741,7 +820,12 @@ int orc_burn(const orc_net_desc *d, int64_t nz, const double *rho, const double 
         for (int i = 0; i < N; i++) srcv[SP(i)] = opts->src_X[(int64_t)i * nz + z] / nt.aion[i];
         srcv[TI] = opts->src_T[z];
       }
-      int code = burn_zone(&nt, rho[z], y0, dt, rtol, atol, opts, has_src ? srcv : NULL, yout, cnt);
+      Trace trc = {NULL, 0, n, 0};
+      const int traced = (z == 0 && opts && opts->trace);
+      if (traced) trc.buf = opts->trace, trc.cap = opts->trace_cap;
+      int code = burn_zone(&nt, rho[z], y0, dt, rtol, atol, opts, has_src ? srcv : NULL, yout, cnt,
+                           traced ? &trc : NULL);
+      if (traced && opts->trace_n) *opts->trace_n = trc.count;
       if (code == -4) { /* invalid input: outputs = inputs */
         for (int i = 0; i < N; i++) X_out[(int64_t)i * nz + z] = X[(int64_t)i * nz + z];
         T_out[z] = T[z];

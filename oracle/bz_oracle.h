@@ -14,11 +14,20 @@
  * SURVEY.md section 8(c) C.1-C.2, and is followed here step by step in that notation.
  *
  * Parity status of the parts (pins live in tests/test_oracle_*.py, all -m "not gpu"):
- *   rate law, RHS, Jacobian, LU/solve, exp/log, BDF coefficients, order of accuracy,
- *   the integrator (closed forms, invariants, brute-force implicit Euler, scipy Radau):
- *   pinned.   The VALUES of the step/order heuristics constants (BIAS1..3, THRESH,
- *   ETAMAX, ...): parity unpinned -- any values pass the pins; they are fixed by
- *   DESIGN.md section 3 only.
+ *   rate law, RHS, Jacobian (incl. every sign of the Y < 0 extension), LU/solve, exp/log, BDF
+ *   coefficients, order of accuracy, the integrator as a whole (closed forms, invariants,
+ *   brute-force implicit Euler, scipy Radau): pinned.
+ *   Step/order machinery (tests/test_oracle_nordsieck.py): build_d against numpy's polyfromroots;
+ *   the Nordsieck array after every accepted step, after both order changes of C.2-E, after the
+ *   order reduction and the order-1 restart of C.2-B.5 = the array of the polynomial that
+ *   interpolates the accepted values, rebuilt in exact rational arithmetic from the trace hook;
+ *   E-, E+ and dsm against analytic derivatives (constant step) and against divided differences
+ *   of the accepted values (variable steps); failure codes -1 (real inputs), -2, -3 (limits as
+ *   parameters).  Each of these pins was checked to turn red under a perturbation of the line it
+ *   covers (commit message of the pins).
+ *   PARITY UNPINNED: only the VALUES of the heuristics constants (BIAS1..3, THRESH, ETAMAX, ETAMIN,
+ *   ETAMXF, ETACF, NTOL, CRDOWN, RDIV, ADDON, SLIVER, the default limits) -- any values pass the
+ *   pins; they are fixed by DESIGN.md section 3 only.
  */
 #ifndef BZ_ORACLE_H
 #define BZ_ORACLE_H
@@ -53,7 +62,30 @@ typedef struct {
    * dY_i/dt += src_X[i][z] / A_i (src_X is a mass-fraction rate [1/s]).  NULL = no sources. */
   const double *src_T; /* [nz] or NULL */
   const double *src_X; /* [N][nz] or NULL (both or neither) */
+  /* test hook (pins of C.2-B.5/D/E, tests/test_oracle_nordsieck.py): if trace != NULL, zone 0 writes
+   * one record of ORC_TRACE_HEAD + 12*n doubles per event, at most trace_cap records, and the number
+   * of events into *trace_n.  Record = {kind, t, h_used, q_used, dsm, eta_q, eta_qm1, eta_qp1, E-, E+,
+   * action, eta, h_next, q_next, nef, ncf, Zacc[6][n], Zend[6][n]} with kind 0 = accepted step
+   * (Zacc = Nordsieck array right after C at scale h_used, Zend = after E at scale h_next; t = the new
+   * time), kind 1 = B.5 third error-test failure lowering the order and kind 2 = B.5 restart at
+   * order 1 (Zend = the array the next attempt starts from, at scale h_next, expanded at the OLD time t;
+   * kind 1: Zacc = the same array before its rescale by ETAMIN, at scale h_used).
+   * Rows of Z are in the API order (Y_0..Y_{N-1}, T).  The hook only copies values out; with
+   * fixed_q > 0 it also evaluates (but never applies) the estimators of C.2-D. */
+  double *trace;
+  int32_t trace_cap;
+  int32_t *trace_n;
+  /* limits of C.2 as call parameters (the library's bz_set_limits; CVODE exposes the same three):
+   * accepted steps per zone (code -3), error-test failures per step (code -2), Newton failures per
+   * step (code -1).  <= 0 = the defaults MXSTEP 20000, MXNEF 7, MXNCF 10. */
+  int32_t mxstep, mxnef, mxncf;
+  /* test hook: the attempts of accepted step number inject_step (1-based) fail the error test until
+   * inject_nef failures have been counted, whatever dsm is.  Natural third failures come after two
+   * step reductions that leave the high Nordsieck rows below rounding, where the order reduction of
+   * C.2-B.5 cannot be observed; injected ones keep them large (tests/test_oracle_nordsieck.py). */
+  int32_t inject_step, inject_nef;
 } orc_opts;
+#define ORC_TRACE_HEAD 16
 
 /* counters[8] = {nst, nrhs, njac, nlu, nsolve, netf, ncfn, nfailzones} summed over zones */
 int orc_burn(const orc_net_desc *d, int64_t nz, const double *rho, const double *T,
@@ -73,6 +105,8 @@ void orc_lu_solve(int n, const double *a, const int32_t *ipvt, const double *inv
 /* l[0..q], for step h and history tau[1..5] (tau[0] unused) */
 void orc_bdf_coeffs(int q, double h, const double *tau, double *l);
 double orc_wrms(int n, const double *v, const double *w, int lanes);
+/* d(x) = x^2 prod_{i=1..cnt} (x + xi[i]) = sum_j d[j] x^j (xi[0] unused; d has 8 entries) */
+void orc_build_d(int cnt, const double *xi, double *d);
 int orc_max_threads(void);
 /* test aid: number of row interchanges orc_lu_factor has performed since the last reset */
 unsigned long long orc_interchanges(int reset);

@@ -21,7 +21,15 @@ class _Desc(C.Structure):
 
 class _Opts(C.Structure):
     _fields_ = [("norm_lanes", C.c_int32), ("fixed_q", C.c_int32), ("fixed_h", C.c_double),
-                ("z_init", _dp), ("nthreads", C.c_int32), ("src_T", _dp), ("src_X", _dp)]
+                ("z_init", _dp), ("nthreads", C.c_int32), ("src_T", _dp), ("src_X", _dp),
+                ("trace", _dp), ("trace_cap", C.c_int32), ("trace_n", _ip),
+                ("mxstep", C.c_int32), ("mxnef", C.c_int32), ("mxncf", C.c_int32),
+                ("inject_step", C.c_int32), ("inject_nef", C.c_int32)]
+
+
+TRACE_HEAD = 16
+TRACE_FIELDS = ("kind", "t", "h_used", "q_used", "dsm", "eta_q", "eta_qm1", "eta_qp1", "E_minus", "E_plus",
+                "action", "eta", "h_next", "q_next", "nef", "ncf")
 
 
 _lib = None
@@ -53,6 +61,8 @@ def _L():
         lib.orc_event_counts.argtypes = [C.c_int, C.POINTER(C.c_uint64)]
         lib.orc_interchanges.restype = C.c_uint64
         lib.orc_interchanges.argtypes = [C.c_int]
+        lib.orc_build_d.restype = None
+        lib.orc_build_d.argtypes = [C.c_int, _dp, _dp]
         _lib = lib
     return _lib
 
@@ -100,10 +110,14 @@ def max_threads() -> int:
 
 
 def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fixed_h=0.0, z_init=None,
-         src_T=None, src_X=None):
+         src_T=None, src_X=None, trace=0, mxstep=0, mxnef=0, mxncf=0, inject=(0, 0)):
     """Integrate every zone over dt.  X: [nspec, nz].  Returns (T_out, X_out, nsteps, counters).
     src_T [nz] (K/s) and src_X [nspec, nz] (mass-fraction rate, 1/s): optional constant source terms
-    (dy/dt = f + s, bz_oracle.h); give both or neither."""
+    (dy/dt = f + s, bz_oracle.h); give both or neither.
+    mxstep / mxnef / mxncf: the limits behind the failure codes -3 / -2 / -1 (0 = defaults 20000 / 7 / 10).
+    inject = (step, nef): test hook, the attempts of accepted step `step` fail the error test nef times.
+    trace = capacity in events: zone 0's event records (bz_oracle.h, orc_opts.trace) are returned as a
+    fifth value, a list of dicts with the TRACE_FIELDS plus 'Zacc', 'Zend' ([6, n] arrays, API order)."""
     rho = np.ascontiguousarray(rho, dtype=np.float64)
     T = np.ascontiguousarray(T, dtype=np.float64)
     X = np.ascontiguousarray(X, dtype=np.float64)
@@ -123,13 +137,30 @@ def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fi
         sT = np.ascontiguousarray(src_T, dtype=np.float64)
         sX = np.ascontiguousarray(src_X, dtype=np.float64)
         assert sT.shape == (nz,) and sX.shape == (d.nspec, nz)
+    n = d.nspec + 1
+    tbuf = np.zeros((int(trace), TRACE_HEAD + 12 * n)) if trace else None
+    tn = np.zeros(1, dtype=np.int32)
     opts = _Opts(int(norm_lanes), int(fixed_q), float(fixed_h), _d(zi) if zi is not None else None,
-                 int(nthreads), _d(sT) if sT is not None else None, _d(sX) if sX is not None else None)
+                 int(nthreads), _d(sT) if sT is not None else None, _d(sX) if sX is not None else None,
+                 _d(tbuf) if trace else None, int(trace), _i(tn), int(mxstep), int(mxnef), int(mxncf), int(inject[0]), int(inject[1]))
     rc = _L().orc_burn(C.byref(d), nz, _d(rho), _d(T), _d(X), dt, rtol, atol, _d(T_out), _d(X_out),
                        _i(nsteps), C.byref(opts), cnt)
     if rc != 0:
         raise ValueError(f"orc_burn failed with code {rc}")
-    return T_out, X_out, nsteps, dict(zip(COUNTER_NAMES, (int(c) for c in cnt)))
+    out = (T_out, X_out, nsteps, dict(zip(COUNTER_NAMES, (int(c) for c in cnt))))
+    if not trace:
+        return out
+    if int(tn[0]) > int(trace):
+        raise ValueError(f"trace capacity {trace} too small for {int(tn[0])} events")
+    recs = []
+    for r in tbuf[: int(tn[0])]:
+        e = dict(zip(TRACE_FIELDS, r[:TRACE_HEAD]))
+        for k in ("kind", "q_used", "action", "q_next", "nef", "ncf"):
+            e[k] = int(e[k])
+        e["Zacc"] = r[TRACE_HEAD:TRACE_HEAD + 6 * n].reshape(6, n).copy()
+        e["Zend"] = r[TRACE_HEAD + 6 * n:].reshape(6, n).copy()
+        recs.append(e)
+    return out + (recs,)
 
 
 def rates(net, rho, y, jac=True):
@@ -176,6 +207,15 @@ def bdf_coeffs(q, h, tau):
     out = np.zeros(8)
     _L().orc_bdf_coeffs(int(q), float(h), _d(t), _d(out))
     return out[: q + 1].copy()
+
+
+def build_d(xi):
+    """Coefficients d_0..d_7 of d(x) = x^2 prod_i (x + xi_i) (C.2-E), xi = [xi_1, xi_2, ...]."""
+    x = np.zeros(8)
+    x[1:1 + len(xi)] = xi
+    d = np.zeros(8)
+    _L().orc_build_d(len(xi), _d(x), _d(d))
+    return d
 
 
 def wrms(v, w, lanes=1):
