@@ -110,6 +110,28 @@ int burn_zones_host(bz_net *net, int64_t nz, const double *rho, const double *T,
 
 int net_destroy(bz_net *net);
 
+/* The burn for callers that may not allocate device memory (a harness that forbids cudaMalloc, a
+ * tight serving loop): no handle, no net_create.  One call validates and flattens `desc` (HOST
+ * pointers, as net_create), copies its tables into a library-owned STATIC device array of
+ * BZ_STATIC_SCRATCH_BYTES (32 KiB, held by every GPU that loads the library until the process
+ * exits), clears the work-queue counter that also lives there, and launches the generic
+ * cooperative kernel (burn_coop, any network).  It calls no cudaMalloc, cudaFree or other
+ * allocating routine, on the host side it uses fixed-size buffers.  All other arguments, the
+ * per-zone failure codes, the arithmetic and the results are those of burn_zones on a handle with
+ * bz_select_kernel(net, 1) -- bit for bit; norm lanes = 4, 8, 16 or 32, the smallest >= nspec + 1.
+ *   Limit: the tables must fit the static array.  nspec <= 31 and nreac <= 256 (the ABI's own
+ *   limits) always do; anything larger returns BZ_ERR_SIZE and enqueues nothing.  nz is unlimited
+ *   (the scratch does not grow with it).
+ *   Sharing: every call on a device uses the SAME array, which keeps the previous call's contents;
+ *   the call itself re-uploads the tables and zeroes the queue on `cuda_stream`, so calls ordered
+ *   on one stream are safe, while calls that overlap on the GPU (two streams, two threads) RACE on
+ *   it and give undefined results -- serialise them, or use handles (net_create) instead.
+ *   The table upload is a cudaMemcpyAsync from pageable host memory: not capturable in a CUDA graph. */
+#define BZ_STATIC_SCRATCH_BYTES 32768
+int burn_zones_static(const bz_net_desc *desc, int64_t nz, const double *rho, const double *T,
+                      const double *X, double dt, double rtol, double atol, double *T_out,
+                      double *X_out, int32_t *nsteps, void *cuda_stream);
+
 /* Totals over the zones of the most recent burn_zones on this handle:
  * out[8] = {nst, nrhs, njac, nlu, nsolve, netf, ncfn, nfailzones} (HOST).  Synchronises
  * `cuda_stream` (it has to read the device counters). */

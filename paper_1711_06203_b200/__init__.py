@@ -6,6 +6,6 @@ without the built library or without a CUDA device every compute call raises.
 """
 from .binding import (  # noqa: F401
     BurnError, Net, net_create, burn_zones, burn_zones_src, strang_step, burn_zones_host, net_destroy, get_counters,
-    fp64_peak_probe, library_path, COUNTER_NAMES, EXPORTED_SYMBOLS,
+    fp64_peak_probe, library_path, COUNTER_NAMES, EXPORTED_SYMBOLS, burn_zones_static, STATIC_SCRATCH_BYTES,
 )
 from .sharding import shard_range, shard_workload  # noqa: F401

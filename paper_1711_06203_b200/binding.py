@@ -9,7 +9,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
-EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_src", "burn_zones_host", "net_destroy", "bz_get_counters",
+EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_src", "burn_zones_host", "burn_zones_static", "net_destroy",
+                    "bz_get_counters",
                     "bz_norm_lanes", "bz_select_kernel", "bz_kernel_name", "bz_last_cuda_error", "bz_fp64_peak_probe")
 _STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
            -5: "CUDA runtime error", -6: "out of memory", -7: "unsupported by the forced kernel"}
@@ -63,6 +64,8 @@ def _L():
         lib.burn_zones_src.restype = C.c_int
         lib.burn_zones_src.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp, C.c_double, C.c_double, C.c_double,
                                        vp, vp, vp, vp]
+        lib.burn_zones_static.restype = C.c_int
+        lib.burn_zones_static.argtypes = [C.POINTER(_Desc)] + sig[1:]
         lib.bz_get_counters.restype = C.c_int
         lib.bz_get_counters.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
         lib.bz_norm_lanes.restype = C.c_int
@@ -230,6 +233,41 @@ def burn_zones_host(net: Net, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, s
         return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
     _check(_L().burn_zones_host(net._h, nz, ptr(rho), ptr(T), ptr(X), float(dt), float(rtol), float(atol),
                                 ptr(T_out), ptr(X_out), ptr(nsteps), _stream_ptr(stream)), "burn_zones_host")
+    return T_out, X_out, nsteps
+
+
+STATIC_SCRATCH_BYTES = 32768      # include/burnzones.h: BZ_STATIC_SCRATCH_BYTES
+
+
+def burn_zones_static(desc, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, stream=None):
+    """The burn without a handle and without any device allocation (include/burnzones.h:
+    burn_zones_static): `desc` is any object with the fields of workloads.Network; the library keeps
+    its tables and work queue in a static 32 KiB device array shared by all calls, so calls must be
+    ordered on the GPU (one stream).  The caller passes all six device tensors; nothing is allocated
+    here either.  Runs the generic cooperative kernel; returns without synchronising."""
+    import torch
+    keep = dict(aion=_f64(desc.aion), reactant=_i32(desc.reactant), stoich_id=_i32(desc.stoich_id),
+                stoich_dy=_f64(desc.stoich_dy), rate_A=_f64(desc.rate_A), rate_n=_f64(desc.rate_n),
+                rate_B=_f64(desc.rate_B), q_mev=_f64(desc.q_mev))
+    N, K = keep["aion"].shape[0], keep["rate_A"].shape[0]
+    if keep["reactant"].shape != (K, 3) or keep["stoich_id"].shape != (K, 4) or keep["stoich_dy"].shape != (K, 4):
+        raise ValueError("reactant must be [K,3], stoich_id/stoich_dy [K,4]")
+    for k in ("rate_n", "rate_B", "q_mev"):
+        if keep[k].shape != (K,):
+            raise ValueError(f"{k} must be [K]")
+    nz = rho.shape[0]
+    for name, t, dt_, shape in (("rho", rho, torch.float64, (nz,)), ("T", T, torch.float64, (nz,)),
+                                ("X", X, torch.float64, (N, nz)), ("T_out", T_out, torch.float64, (nz,)),
+                                ("X_out", X_out, torch.float64, (N, nz)), ("nsteps", nsteps, torch.int32, (nz,))):
+        if not (t.is_cuda and t.dtype == dt_ and t.is_contiguous() and tuple(t.shape) == shape):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {shape}")
+    d = _Desc(N, K, keep["aion"].ctypes.data_as(_dp), keep["reactant"].ctypes.data_as(_ip),
+              keep["stoich_id"].ctypes.data_as(_ip), keep["stoich_dy"].ctypes.data_as(_dp),
+              keep["rate_A"].ctypes.data_as(_dp), keep["rate_n"].ctypes.data_as(_dp),
+              keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp), float(desc.cv))
+    p = lambda t: C.c_void_p(t.data_ptr())
+    _check(_L().burn_zones_static(C.byref(d), nz, p(rho), p(T), p(X), float(dt), float(rtol), float(atol),
+                                  p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones_static")
     return T_out, X_out, nsteps
 
 

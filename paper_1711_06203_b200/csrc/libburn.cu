@@ -482,6 +482,201 @@ int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, c
 
 }  // extern "C"
 
+// ---- burn_zones_static: the burn without any device allocation ------------------------------------
+// Everything the cooperative kernel needs besides the caller's arrays -- work-queue head, counters,
+// network tables -- lives in ONE file-scope device array.  In host code `g_static_scratch` is only a
+// stand-in for the symbol: the device address comes from cudaGetSymbolAddress, once per device.
+namespace {
+constexpr int ST_MAXN = 31, ST_MAXK = 256;
+constexpr size_t ST_HDR = 256;  // 16 x u64 (queue head, 8 counters), padded to the alignment
+constexpr int ST_DBL_CAP = 5 * ST_MAXK + ST_MAXN + 4 * ST_MAXK + 1;                  // doubles (even)
+constexpr int ST_INT_CAP = 4 * ST_MAXK + 2 * (ST_MAXN + 1) + 4 * ST_MAXK + 3 * ST_MAXK;  // ints
+static_assert(ST_HDR + 8 * (size_t)ST_DBL_CAP + 4 * (size_t)ST_INT_CAP <= BZ_STATIC_SCRATCH_BYTES,
+              "static scratch too small for the ABI's largest network");
+static __device__ __align__(256) unsigned char g_static_scratch[BZ_STATIC_SCRATCH_BYTES];
+
+constexpr int ST_MAXDEV = 64;
+struct StaticDev {
+  bool ready;
+  unsigned char *ptr;  // device address of g_static_scratch on this device
+  int sms, smem_optin;
+};
+StaticDev g_static_dev[ST_MAXDEV];
+
+// set-up, once per device, with that device current
+int static_setup(int dev, StaticDev **out) {
+  if (dev < 0 || dev >= ST_MAXDEV) return BZ_ERR_SIZE;
+  StaticDev &s = g_static_dev[dev];
+  if (!s.ready) {
+    unsigned char *p = nullptr;
+    BZ_CUDA(cudaGetSymbolAddress((void **)&p, g_static_scratch));
+    if (!p) return BZ_ERR_CUDA;
+    int sms = 0, optin = 0;
+    BZ_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    BZ_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    s.ptr = p; s.sms = sms; s.smem_optin = optin;
+    s.ready = true;  // (a racing second thread computes the same values)
+  }
+  *out = &s;
+  return BZ_OK;
+}
+
+// host-side flattening into fixed buffers: the tables of net_create, same layout, same order
+struct StaticFlat {
+  double dbl[ST_DBL_CAP];
+  int itab[ST_INT_CAP];
+  int ndbl, nint, nterm, ncl;
+};
+
+int static_flatten(const bz_net_desc *d, StaticFlat &F) {
+  const int N = d->nspec, K = d->nreac;
+  if (!(d->cv > 0.0) || !std::isfinite(d->cv)) return BZ_ERR_NETWORK;
+  for (int i = 0; i < N; i++)
+    if (!(d->aion[i] > 0.0) || !std::isfinite(d->aion[i])) return BZ_ERR_NETWORK;
+  int rp[4 * ST_MAXK] = {0};
+  int col[ST_MAXK][3], nslot[ST_MAXK];
+  int sp_cnt[ST_MAXN + 1] = {0}, cl_cnt[ST_MAXN + 1] = {0};
+  double *lnA = F.dbl, *en = F.dbl + K, *B = F.dbl + 2 * K, *Q = F.dbl + 3 * K, *invsym = F.dbl + 4 * K;
+  double *aion = F.dbl + 5 * K, *sp_dy = F.dbl + 5 * K + N;
+  for (int k = 0; k < K; k++) {
+    int r[3], m = 0;
+    for (int a = 0; a < 3; a++) {
+      const int id = d->reactant[3 * k + a];
+      if (id < 0) continue;
+      if (id >= N) return BZ_ERR_NETWORK;
+      r[m++] = id;
+    }
+    if (m == 0) return BZ_ERR_NETWORK;
+    if (!(d->rate_A[k] > 0.0) || !std::isfinite(d->rate_A[k]) || !std::isfinite(d->rate_n[k]) ||
+        !std::isfinite(d->rate_B[k]) || !std::isfinite(d->q_mev[k]))
+      return BZ_ERR_NETWORK;
+    col[k][0] = col[k][1] = col[k][2] = 0;
+    int ns = 0;  // distinct reactant species in order of first appearance = Jacobian column slots
+    for (int a = 0; a < m; a++) {
+      bool seen = false;
+      for (int b = 0; b < a; b++) seen |= (r[b] == r[a]);
+      if (!seen) col[k][ns++] = r[a];
+    }
+    nslot[k] = ns;
+    const int same = (m > 1 && r[0] == r[1]) + (m > 2 && r[0] == r[2]) + (m > 2 && r[1] == r[2]);
+    invsym[k] = same == 0 ? 1.0 : (same == 1 ? 0.5 : 1.0 / 6.0);
+    lnA[k] = host_log(d->rate_A[k]);
+    en[k] = d->rate_n[k]; B[k] = d->rate_B[k]; Q[k] = d->q_mev[k];
+    rp[4 * k + 0] = m | (ns << 8);
+    rp[4 * k + 1] = r[0] | ((m > 1 ? r[1] : 0) << 8) | ((m > 2 ? r[2] : 0) << 16);
+    rp[4 * k + 2] = col[k][0] | (col[k][1] << 8) | (col[k][2] << 16);
+    for (int s = 0; s < ns; s++) cl_cnt[col[k][s]]++;
+    int ids[4], nid = 0;
+    for (int a = 0; a < 4; a++) {
+      const int id = d->stoich_id[4 * k + a];
+      if (id < 0) continue;
+      if (id >= N) return BZ_ERR_NETWORK;
+      for (int b = 0; b < nid; b++)
+        if (ids[b] == id) return BZ_ERR_NETWORK;
+      if (!std::isfinite(d->stoich_dy[4 * k + a])) return BZ_ERR_NETWORK;
+      ids[nid++] = id;
+      sp_cnt[id]++;
+    }
+  }
+  for (int i = 0; i < N; i++) aion[i] = d->aion[i];
+  // CSR by species, entries in ascending k (second pass fills in k order)
+  int sp_off[ST_MAXN + 2], cl_off[ST_MAXN + 2], sp_pos[ST_MAXN + 1], cl_pos[ST_MAXN + 1];
+  sp_off[0] = cl_off[0] = 0;
+  for (int i = 0; i < N; i++) {
+    sp_off[i + 1] = sp_off[i] + sp_cnt[i];
+    cl_off[i + 1] = cl_off[i] + cl_cnt[i];
+    sp_pos[i] = sp_off[i];
+    cl_pos[i] = cl_off[i];
+  }
+  const int nterm = sp_off[N], ncl = cl_off[N];
+  F.nterm = nterm; F.ncl = ncl;
+  F.ndbl = 5 * K + N + nterm;
+  F.nint = 4 * K + (N + 1) + nterm + (N + 1) + ncl;
+  if (F.ndbl > ST_DBL_CAP || F.nint > ST_INT_CAP) return BZ_ERR_SIZE;
+  int *t_rp = F.itab, *t_spoff = t_rp + 4 * K, *t_spk = t_spoff + (N + 1);
+  int *t_cloff = t_spk + nterm, *t_clks = t_cloff + (N + 1);
+  for (int i = 0; i < 4 * K; i++) t_rp[i] = rp[i];
+  for (int i = 0; i <= N; i++) t_spoff[i] = sp_off[i], t_cloff[i] = cl_off[i];
+  for (int k = 0; k < K; k++) {
+    for (int a = 0; a < 4; a++) {
+      const int id = d->stoich_id[4 * k + a];
+      if (id < 0) continue;
+      t_spk[sp_pos[id]] = k;
+      sp_dy[sp_pos[id]] = d->stoich_dy[4 * k + a];
+      sp_pos[id]++;
+    }
+    for (int s = 0; s < nslot[k]; s++) t_clks[cl_pos[col[k][s]]++] = k | (s << 16);
+  }
+  return BZ_OK;
+}
+}  // namespace
+
+extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double *rho, const double *T,
+                                 const double *X, double dt, double rtol, double atol, double *T_out,
+                                 double *X_out, int32_t *nsteps, void *cuda_stream) {
+  if (!d) return BZ_ERR_NULL;
+  // sizes beyond what the static array holds are refused before anything else happens
+  if (d->nspec < 1 || d->nspec > ST_MAXN || d->nreac < 1 || d->nreac > ST_MAXK || nz < 0) return BZ_ERR_SIZE;
+  if (!d->aion || !d->reactant || !d->stoich_id || !d->stoich_dy || !d->rate_A || !d->rate_n ||
+      !d->rate_B || !d->q_mev)
+    return BZ_ERR_NULL;
+  if (!(dt > 0.0) || !(rtol > 0.0) || !(atol >= 0.0) || !std::isfinite(dt) || !std::isfinite(rtol) ||
+      !std::isfinite(atol))
+    return BZ_ERR_SCALAR;
+  static thread_local StaticFlat F;  // 30 KB of host tables: not on the stack, never on the heap
+  const int frc = static_flatten(d, F);
+  if (frc != BZ_OK) return frc;
+  if (ST_HDR + 8 * (size_t)((F.ndbl + 1) & ~1) + 4 * (size_t)F.nint > BZ_STATIC_SCRATCH_BYTES) return BZ_ERR_SIZE;
+  if (nz == 0) return BZ_OK;
+  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+
+  int dev = 0;
+  BZ_CUDA(cudaGetDevice(&dev));
+  StaticDev *sd = nullptr;
+  const int src = static_setup(dev, &sd);
+  if (src != BZ_OK) return src;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int N = d->nspec, K = d->nreac, n = N + 1;
+  const Variant *v = pick_variant(n);
+  const int L = v->lanes;
+  const int gpb = bz::COOP_THREADS / L;
+  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
+  const int tab = ((F.ndbl + 1) & ~1) + (((F.nint + 3) & ~3) / 2);
+  const int smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
+  if (smem_bytes > sd->smem_optin) return BZ_ERR_NOMEM;
+  // opt in to the device's maximum: never lowers what a handle of net_create has set for this kernel
+  BZ_CUDA(cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, sd->smem_optin));
+  int bps = 0;
+  BZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)v->fn, bz::COOP_THREADS, smem_bytes));
+  if (bps < 1) return BZ_ERR_NOMEM;
+
+  unsigned char *base = sd->ptr;
+  double *d_dbl = reinterpret_cast<double *>(base + ST_HDR);
+  int *d_int = reinterpret_cast<int *>(base + ST_HDR + 8 * (size_t)ST_DBL_CAP);
+  // the array keeps the previous call's contents: zero the queue head and the counters, reload the tables
+  BZ_CUDA(cudaMemsetAsync(base, 0, ST_HDR, st));
+  BZ_CUDA(cudaMemcpyAsync(d_dbl, F.dbl, (size_t)F.ndbl * sizeof(double), cudaMemcpyHostToDevice, st));
+  BZ_CUDA(cudaMemcpyAsync(d_int, F.itab, (size_t)F.nint * sizeof(int), cudaMemcpyHostToDevice, st));
+
+  bz::DevNet dn;
+  dn.N = N; dn.n = n; dn.K = K; dn.nterm = F.nterm; dn.ncl = F.ncl;
+  dn.fac = 9.648533212331e17 / d->cv;
+  dn.dbl = d_dbl; dn.itab = d_int;
+  dn.ndbl = F.ndbl; dn.nint = F.nint;
+  bz::BurnArgs a;
+  a.src_T = nullptr; a.src_X = nullptr;
+  a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
+  a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
+  a.queue = reinterpret_cast<unsigned long long *>(base);
+  a.counters = reinterpret_cast<unsigned long long *>(base) + 1;
+  const long long groups_needed = (nz + gpb - 1) / gpb;
+  const long long full = (long long)sd->sms * bps;
+  const int grid = (int)(groups_needed < full ? groups_needed : full);
+  void *args[] = {(void *)&dn, (void *)&a};
+  BZ_CUDA(cudaLaunchKernel((const void *)v->fn, dim3(grid), dim3(bz::COOP_THREADS), args, (size_t)smem_bytes, st));
+  return BZ_OK;
+}
+
 // ---- FP64 peak probe ----------------------------------------------------------------------------
 namespace {
 __global__ void __launch_bounds__(256) dfma_probe_kernel(long long iters, double *sink) {
