@@ -2,11 +2,14 @@
 """bench.py -- zones burned/sec on the 13-isotope 128^3 config (BASELINE.json configs[2]).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+                    [--static-schedule] [--kernel auto|coop|quad]
 
 A "step" is one pass of the whole hot path (a1-a9: load, work queue, rates, Jacobian, LU,
 Newton, BDF control, store) over one batch of synthetic zones: one burn_zones call.
-N > 1: one process per GPU (torchrun), every rank burns its own copy of the config (weak
-scaling, no data-path collective); value = zones of all ranks / max time.
+N > 1: one process per GPU, every rank burns its own copy of the config (weak scaling, no data-path
+collective); value = zones of all ranks / max time.  Started under torchrun the
+ranks are used as given; started plainly with --gpus N > 1 the script re-launches itself under
+torch.distributed.run with N ranks on 127.0.0.1.
 Prints ONE JSON line on rank 0.  DESIGN.md section 6 defines every field.
 """
 import argparse
@@ -29,6 +32,7 @@ METRIC = "zones burned/sec (13-isotope net, fp64 BDF)"
 UNIT = "zones/s"
 FP64_LANES_PER_SM = 64           # DFMA lanes per SM
 CPU_SAMPLE_STRIDE = {1: 1, 2: 16, 3: 64, 4: 64, 5: 512}
+SINGLE_CORE_STRIDE = {1: 1, 2: 128, 3: 1024, 4: 8192, 5: 4096}   # <= 4096 zones, one thread (the axis of PAPER.md:L127 Fig. 5)
 
 
 def _workload_name(cfg):
@@ -100,6 +104,47 @@ def run_reference(args):
     }))
 
 
+def _max_over_ranks(values, device, world):
+    """Timings are reported as the MAX over ranks (the job is done when its slowest rank is)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def run_stub(args):
+    """--stub (tests only, tests/test_bench_launcher.py): the multi-rank plumbing of run_ours --
+    rendezvous, barrier, max-over-ranks timing, one JSON line from rank 0 -- with the gloo backend and a
+    sleep in place of the burn, so that the N > 1 path can be exercised on a box without GPUs."""
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    nz = 1000
+    for _ in range(args.warmup):
+        time.sleep(0.001)
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time.sleep(0.01 * (rank + 1))            # rank r is (r + 1) x slower: the max must win
+    total_ms = (time.perf_counter() - t0) * 1e3
+    if world > 1:
+        dist.barrier()
+    (total_ms,) = _max_over_ranks([total_ms], torch.device("cpu"), world)
+    if rank == 0:
+        ms = total_ms / args.steps
+        print(json.dumps({"metric": METRIC, "value": world * nz / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "stub": True,
+                          "scaling": "weak", "config": {"workload": "stub (sleep)", "zones_per_gpu": nz}}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -117,10 +162,12 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = args.config
-    w = make_workload(cfg)                       # every rank burns its own full copy (weak scaling)
+    # every rank burns its own full copy (weak scaling); --stride S (profiling only) = every S-th zone
+    w = make_workload(cfg, zones=args.stride if args.stride > 1 else None)
     nz, N = w.nz, w.net.nspec
     net = bz.net_create(w.net)
     net.select_kernel(args.kernel)
+    net.set_schedule("static" if args.static_schedule else "queue")
     stream = torch.cuda.current_stream()
 
     # ---- device-resident arm -------------------------------------------------------------------
@@ -173,10 +220,7 @@ def run_ours(args):
     same = bool(np.array_equal(Xo_h.numpy(), Xo_d.cpu().numpy()))
 
     # ---- max over ranks ------------------------------------------------------------------------
-    tms = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(tms[0]), float(tms[1])
+    total_ms, e2e_ms = _max_over_ranks([total_ms, e2e_ms], dev, world)
     ms_per_step = total_ms / args.steps
     value = world * nz / (ms_per_step * 1e-3)
     e2e_value = world * nz / (e2e_ms * 1e-3)
@@ -196,23 +240,36 @@ def run_ours(args):
         kern_ms = float(np.mean(per_launch_ms))
         achieved = aflops / (kern_ms * 1e-3) / 1e12
         sbytes = state_bytes_per_zone(N)
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")      # written from an ncu --set full capture
+        # two figures that only a profiler can give are COPIED from the committed ncu summaries of this
+        # kernel on this config (profiles/ncu_counters.json names the capture); null when none exists
+        traffic = executed = None
+        ncu_src = None
+        tpath = os.path.join(ROOT, "profiles", "ncu_counters.json")
         if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get(f"config{cfg}:{net.kernel_name}")
+            rec = json.load(open(tpath)).get(f"config{cfg}:{net.kernel_name}")
+            if rec and not args.static_schedule:
+                traffic, executed, ncu_src = rec.get("dram_bytes"), rec.get("executed_fp64_flops"), rec.get("source")
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(cfg), "zones_per_gpu": nz, "neq": N + 1, "nreac": w.net.nreac,
+            "config": {"workload": _workload_name(cfg) + (f", every {args.stride}th zone" if args.stride > 1 else ""),
+                       "zones_per_gpu": nz, "neq": N + 1, "nreac": w.net.nreac,
                        "dt": w.dt, "rtol": w.rtol, "atol": w.atol, "kernel": net.kernel_name,
-                       "l2": f"inputs {8 * (N + 2) * nz / 1e6:.0f} MB per step exceed the 126 MB L2",
+                       "schedule": "static round-robin (a2 off)" if args.static_schedule else "work queue (a2)",
+                       "l2": (f"inputs {8 * (N + 2) * nz / 1e6:.0f} MB per step exceed the 126 MB L2" if 8 * (N + 2) * nz > 126e6
+                              else f"inputs {8 * (N + 2) * nz / 1e6:.1f} MB per step fit the L2; the kernel is ALU-bound, "
+                                   "state traffic is < 1e-3 of its time"),
                        "parallelism": f"zones sharded, {world} replica(s), no collective"},
             "rhs_evals_per_s": world * counters["nrhs"] / (kern_ms * 1e-3),
             "steps_per_zone_mean": counters["nst"] / nz, "failed_zones": nfail, "counters": counters,
             "hbm_state_gbs": sbytes * nz / (kern_ms * 1e-3) / 1e9,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": traffic,
+                         "traffic_source": ncu_src,
+                         # FP64 flops the kernel EXECUTES per launch (ncu dadd + dmul + 2 dfma thread instructions,
+                         # same capture) over the live kernel time: redundant lanes included, unlike `frac`
+                         "executed_frac": (executed / (kern_ms * 1e-3) / 1e12 / peak_tf) if executed else None,
                          "peak_source": f"{props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
                                         f"{sm_max_mhz:.0f} MHz (derived); DFMA probe measured {probe_tf:.2f} TFLOP/s",
                          "frac_of_measured_probe": achieved / probe_tf,
@@ -232,10 +289,32 @@ def run_ours(args):
             el = time.perf_counter() - t0
             out["cpu_baseline"] = {"value": ws.nz / el, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
                                    "sample": f"every {stride}th zone ({ws.nz} zones), {el:.1f} s wall"}
+            s1 = SINGLE_CORE_STRIDE[cfg]
+            w1 = make_workload(cfg, zones=s1 if s1 > 1 else None)
+            t0 = time.perf_counter()
+            oracle.burn(w1.net, w1.rho, w1.T, w1.X, w1.dt, w1.rtol, w1.atol, nthreads=1)
+            el1 = time.perf_counter() - t0
+            out["cpu_baseline"]["single_core"] = {"value": w1.nz / el1, "unit": UNIT, "cores": 1,
+                                                  "sample": f"every {s1}th zone ({w1.nz} zones), {el1:.1f} s wall"}
         print(json.dumps(out))
     bz.net_destroy(net)
     if world > 1:
         dist.destroy_process_group()
+
+
+def relaunch(n, argv, extra_env=None):
+    """`python bench.py --gpus N` without torchrun: start N ranks of this script on this node
+    (one per GPU, rendezvous on 127.0.0.1) and hand their exit code back."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    env.update(extra_env or {})
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -246,10 +325,24 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "coop", "tpz", "quad"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "coop", "quad"],
                     help="auto = specialised quad kernel when the topology has one, else the generic coop kernel")
+    ap.add_argument("--static-schedule", action="store_true",
+                    help="switch the work queue (step a2) off: static round-robin zone assignment, for the before/after figure")
+    ap.add_argument("--stride", type=int, default=1,
+                    help="burn every S-th zone of the config only (short ncu captures; not a bench value)")
+    ap.add_argument("--stub", action="store_true", help=argparse.SUPPRESS)   # tests only: see run_stub
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    world = os.environ.get("WORLD_SIZE")
+    if world is None and args.gpus > 1:
+        sys.exit(relaunch(args.gpus, sys.argv[1:]))
+    if world is not None and int(world) != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with --nproc-per-node {args.gpus}")
+    if args.stub:
+        run_stub(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

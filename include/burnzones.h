@@ -41,7 +41,8 @@ typedef enum {
   BZ_ERR_SCALAR = -4,  /* dt <= 0, rtol <= 0, atol < 0, or non-finite                         */
   BZ_ERR_CUDA = -5,    /* CUDA runtime error; the cudaError_t is in bz_last_cuda_error()      */
   BZ_ERR_NOMEM = -6,   /* host or device allocation failed                                    */
-  BZ_ERR_UNSUPPORTED = -7 /* the kernel forced with bz_select_kernel cannot do what was asked     */
+  BZ_ERR_UNSUPPORTED = -7, /* reserved (was: the forced kernel cannot do what was asked)           */
+  BZ_ERR_DEVICE = -8   /* the handle was created on another device than the current one        */
 } bz_status;
 
 /* Network descriptor.  All pointers are HOST pointers and are
@@ -62,7 +63,10 @@ typedef struct {
   double cv;                 /* specific heat, erg g^-1 K^-1, constant                         */
 } bz_net_desc;
 
-/* Validate, flatten and upload a network.  *out receives the handle. */
+/* Validate, flatten and upload a network.  *out receives the handle.  A handle belongs to the
+ * device that is current when net_create runs (its tables, scratch, grid size and shared-memory
+ * opt-in live there): create one handle per device; every later call on it checks cudaGetDevice
+ * and returns BZ_ERR_DEVICE, enqueuing nothing, if another device is current. */
 int net_create(const bz_net_desc *desc, bz_net **out);
 
 /* Integrate every zone's network over [0, dt] (steps a1-a9 of DESIGN.md section 2).
@@ -94,9 +98,8 @@ int burn_zones(const bz_net *net, int64_t nz, const double *rho, const double *T
  * Both NULL: identical to burn_zones (bit for bit).  Exactly one NULL: BZ_ERR_NULL.  The sources
  * enter every right-hand-side evaluation as one rounded addition after the network's own sums;
  * the Jacobian is unchanged.  A zone with a non-finite source ends with code -4.  All other
- * arguments, the failure codes and the execution rules are those of burn_zones.  Served by the
- * cooperative and the quad kernels; with the thread-per-zone kernel forced (bz_select_kernel
- * kind 2) the call returns BZ_ERR_UNSUPPORTED.  (DESIGN.md section 10.) */
+ * arguments, the failure codes and the execution rules are those of burn_zones.  Served by both
+ * kernels.  (DESIGN.md section 10.) */
 int burn_zones_src(const bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
                    const double *src_T, const double *src_X, double dt, double rtol, double atol,
                    double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream);
@@ -144,10 +147,22 @@ int bz_norm_lanes(const bz_net *net);
 
 /* Kernel selection: kind 0 = automatic (the network-specialised 4-lanes-per-zone kernel if the
  * topology has one compiled in, else the generic cooperative kernel), 1 = always the generic
- * cooperative kernel, 2 = the specialised thread-per-zone kernel, 3 = the specialised quad
- * kernel (2 and 3 fall back to the cooperative kernel when the topology has none).  All follow
- * the same arithmetic; only bz_norm_lanes differs. */
+ * cooperative kernel, 3 = the specialised quad kernel (falls back to the cooperative kernel when
+ * the topology has none); other values: BZ_ERR_SIZE.  Both follow the same arithmetic; only
+ * bz_norm_lanes differs. */
 int bz_select_kernel(bz_net *net, int kind);
+
+/* Zone scheduling (step a2, "a lot of thread divergence due to the widely differing thermodynamic
+ * conditions"): kind 0 (default) = a global work queue -- a lane group that finishes
+ * its zone fetches the next one, so co-resident zones never wait for the slowest of a fixed batch;
+ * kind 1 = static round-robin assignment (group g burns zones g, g + G, g + 2G, ...), kept only so
+ * that the benefit of the queue can be MEASURED (bench.py --static-schedule).  Results are identical. */
+int bz_set_schedule(bz_net *net, int kind);
+
+/* Limits behind the per-zone failure codes: accepted steps (-3), error-test failures on one step
+ * (-2), Newton failures on one step (-1).  0 keeps the default (20000, 7, 10); negative: BZ_ERR_SIZE.
+ * (CVODE exposes the same three; DESIGN.md 3.8 reading s29.) */
+int bz_set_limits(bz_net *net, int32_t mxstep, int32_t mxnef, int32_t mxncf);
 
 /* Name of the kernel variant burn_zones launches for this network (static string). */
 const char *bz_kernel_name(const bz_net *net);

@@ -37,6 +37,9 @@
 #define ETAMAX 2.0
 #define MXSTEP 20000
 #define SLIVER 1e-6
+/* policy 1 ("BZ-BDF v2": VODE's Newton-matrix reuse, ref. [33] PAPER.md:L184) */
+#define CCMAX 0.3 /* refactor when |gamma/gamma_P - 1| exceeds this */
+#define MSBP 20   /* ... or when this many steps were accepted since the last factorisation */
 
 static const double FACT[8] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0, 720.0, 5040.0};
 static const double INVP[8] = {0.0, 1.0, 1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0, 1.0 / 6.0, 1.0 / 7.0};
@@ -428,6 +431,10 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
   const int mxstep = (o && o->mxstep > 0) ? o->mxstep : MXSTEP;
   const int mxnef = (o && o->mxnef > 0) ? o->mxnef : MXNEF;
   const int mxncf = (o && o->mxncf > 0) ? o->mxncf : MXNCF;
+  /* policy 1: the LU of P = I - gamma_P J is KEPT across steps (P, inv, ipvt below persist) */
+  const int reuse = (o && o->policy == 1);
+  double gamP = 0.0;
+  int nslp = 0, haveP = 0, forceP = 0;
   double Z[QMAX + 2][ORC_NMAX], S[ORC_NMAX], w[ORC_NMAX], acor[ORC_NMAX], y[ORC_NMAX];
   double f[ORC_NMAX], b[ORC_NMAX], vtmp[ORC_NMAX];
   double P[ORC_NMAX * ORC_NMAX], inv[ORC_NMAX];
@@ -504,14 +511,40 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
       predict(n, q, Z); /* B.2 */
       predicted = 1;
       for (int i = 0; i < n; i++) y[i] = Z[0][i];
+      int jcur = 1, tried = 0; /* jcur: P was factorised in THIS attempt (always, under policy 0) */
       if (!invalid_state(n, y)) { /* B.3 */
-        rates(nt, rho, y, f, P);
-        add_source(n, src, f);
-        cnt[1]++, cnt[2]++;
-        for (int i = 0; i < n; i++)
-          for (int j = 0; j < n; j++) P[i * n + j] = fma(-gamma, P[i * n + j], (i == j) ? 1.0 : 0.0);
-        int info = orc_lu_factor(n, P, ipvt, inv);
-        cnt[3]++;
+        tried = 1;
+        int needP = 1;
+        if (reuse) {
+          /* policy 1, B.3': factorise only if there is no P yet, a failure asked for it, gamma has
+           * drifted more than CCMAX from gamma_P, or MSBP steps were accepted since */
+          /* |gamma/gamma_P - 1| > CCMAX written without a division: gl = gamma_P l_1 ( = h_P l_1/l_1P ) */
+          const double gl = gamP * l1;
+          needP = !haveP || forceP || fabs(h - gl) > CCMAX * gl || (nst - nslp >= MSBP);
+        }
+        int info = 0;
+        if (needP) {
+          rates(nt, rho, y, f, P);
+          add_source(n, src, f);
+          cnt[1]++, cnt[2]++;
+          for (int i = 0; i < n; i++)
+            for (int j = 0; j < n; j++) P[i * n + j] = fma(-gamma, P[i * n + j], (i == j) ? 1.0 : 0.0);
+          info = orc_lu_factor(n, P, ipvt, inv);
+          cnt[3]++;
+          gamP = gamma, nslp = nst, haveP = !info, forceP = 0;
+        } else {
+          rates(nt, rho, y, f, NULL);
+          add_source(n, src, f);
+          cnt[1]++;
+          jcur = 0;
+        }
+        /* policy 1: every correction solved with a STALE matrix is scaled by 2/(1 + gamma/gamma_P), written
+         * as 2 gl/(gl + h) with gl = gamma_P l_1 (one division that does not wait for gamma = h/l_1) */
+        double cscale = 1.0;
+        if (reuse && !jcur) {
+          const double gl = gamP * l1;
+          cscale = (2.0 * gl) / (gl + h);
+        }
         if (!info) { /* B.4 Newton */
           for (int i = 0; i < n; i++) acor[i] = 0.0;
           double crate = 1.0, delp = 0.0;
@@ -527,6 +560,8 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
             for (int i = 0; i < n; i++) b[i] = fma(gamma, f[i], -fma(Z[1][i], rl1, acor[i]));
             orc_lu_solve(n, P, ipvt, inv, b);
             cnt[4]++;
+            if (reuse && !jcur)
+              for (int i = 0; i < n; i++) b[i] = b[i] * cscale;
             for (int i = 0; i < n; i++) acor[i] = acor[i] + b[i];
             double del = orc_wrms(n, b, w, L);
             if (!isfinite(del)) break;
@@ -545,7 +580,15 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
           }
         }
       }
+      if (!ok && reuse && tried && !jcur) {
+        /* policy 1, B.6': Newton failed with a STALE matrix: same step, same h, fresh J and LU */
+        retract(n, q, Z);
+        forceP = 1;
+        if (o->nstale) __atomic_fetch_add(o->nstale, 1ull, __ATOMIC_RELAXED);
+        continue;
+      }
       if (!ok) { /* B.6 Newton failure */
+        forceP = 1;
         if (predicted) retract(n, q, Z);
         ncf++, cnt[6]++;
         etamax = 1.0;
@@ -566,6 +609,7 @@ static int burn_zone(const Net *nt, double rho, const double *y0, double dt, dou
       nef++, cnt[5]++;
       etamax = 1.0;
       last = 0;
+      forceP = 1; /* policy 1: the retry after an error-test failure uses a fresh matrix */
       if (nef == mxnef) {
         for (int i = 0; i < n; i++) yout[i] = Z[0][i];
         return -2;

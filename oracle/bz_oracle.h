@@ -84,6 +84,18 @@ typedef struct {
    * step reductions that leave the high Nordsieck rows below rounding, where the order reduction of
    * C.2-B.5 cannot be observed; injected ones keep them large (tests/test_oracle_nordsieck.py). */
   int32_t inject_step, inject_nef;
+  /* Newton-matrix policy.  0 ("BZ-BDF v1", the default and the parity reference of burn_zones): a
+   * fresh Jacobian and LU on every attempt.  1 ("BZ-BDF v2", the library's bz_set_policy(net, 1);
+   * VODE's reuse, ref. [33] PAPER.md:L184): the LU of
+   * P = I - gamma_P J is kept; an attempt factorises (with a fresh J at the prediction) only if there is
+   * no P yet, or |gamma/gamma_P - 1| > 0.3, or 20 steps were accepted since, or a failure asked for
+   * it; otherwise it evaluates f only and every correction solved with the stale matrix is multiplied
+   * by 2/(1 + gamma/gamma_P).  Evaluation (part of the contract): gl = gamma_P * l_1; drift test
+   * |h - gl| > 0.3 * gl; scale (2 * gl)/(gl + h).  A Newton failure with a stale matrix repeats the attempt at the same h
+   * with a fresh one (counted in *nstale, not in ncfn); any B.5 or B.6 failure forces a fresh matrix
+   * for the retry (a reduced step of 0.7-0.74 h would not trip the drift test by itself). */
+  int32_t policy;
+  unsigned long long *nstale; /* test aid: stale-matrix retries, summed over zones; or NULL */
 } orc_opts;
 #define ORC_TRACE_HEAD 16
 

@@ -24,7 +24,8 @@ class _Opts(C.Structure):
                 ("z_init", _dp), ("nthreads", C.c_int32), ("src_T", _dp), ("src_X", _dp),
                 ("trace", _dp), ("trace_cap", C.c_int32), ("trace_n", _ip),
                 ("mxstep", C.c_int32), ("mxnef", C.c_int32), ("mxncf", C.c_int32),
-                ("inject_step", C.c_int32), ("inject_nef", C.c_int32)]
+                ("inject_step", C.c_int32), ("inject_nef", C.c_int32),
+                ("policy", C.c_int32), ("nstale", C.POINTER(C.c_uint64))]
 
 
 TRACE_HEAD = 16
@@ -110,11 +111,13 @@ def max_threads() -> int:
 
 
 def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fixed_h=0.0, z_init=None,
-         src_T=None, src_X=None, trace=0, mxstep=0, mxnef=0, mxncf=0, inject=(0, 0)):
+         src_T=None, src_X=None, trace=0, mxstep=0, mxnef=0, mxncf=0, inject=(0, 0), policy=0):
     """Integrate every zone over dt.  X: [nspec, nz].  Returns (T_out, X_out, nsteps, counters).
     src_T [nz] (K/s) and src_X [nspec, nz] (mass-fraction rate, 1/s): optional constant source terms
     (dy/dt = f + s, bz_oracle.h); give both or neither.
     mxstep / mxnef / mxncf: the limits behind the failure codes -3 / -2 / -1 (0 = defaults 20000 / 7 / 10).
+    policy: 0 = fresh Jacobian and LU on every attempt (v1, default); 1 = VODE-style reuse of the Newton
+    matrix (v2, bz_oracle.h); with policy 1 the counters dict also holds 'nstale'.
     inject = (step, nef): test hook, the attempts of accepted step `step` fail the error test nef times.
     trace = capacity in events: zone 0's event records (bz_oracle.h, orc_opts.trace) are returned as a
     fifth value, a list of dicts with the TRACE_FIELDS plus 'Zacc', 'Zend' ([6, n] arrays, API order)."""
@@ -140,14 +143,18 @@ def burn(net, rho, T, X, dt, rtol, atol, norm_lanes=1, nthreads=0, fixed_q=0, fi
     n = d.nspec + 1
     tbuf = np.zeros((int(trace), TRACE_HEAD + 12 * n)) if trace else None
     tn = np.zeros(1, dtype=np.int32)
+    stale = C.c_uint64(0)
     opts = _Opts(int(norm_lanes), int(fixed_q), float(fixed_h), _d(zi) if zi is not None else None,
                  int(nthreads), _d(sT) if sT is not None else None, _d(sX) if sX is not None else None,
-                 _d(tbuf) if trace else None, int(trace), _i(tn), int(mxstep), int(mxnef), int(mxncf), int(inject[0]), int(inject[1]))
+                 _d(tbuf) if trace else None, int(trace), _i(tn), int(mxstep), int(mxnef), int(mxncf), int(inject[0]), int(inject[1]),
+                 int(policy), C.cast(C.pointer(stale), C.POINTER(C.c_uint64)))
     rc = _L().orc_burn(C.byref(d), nz, _d(rho), _d(T), _d(X), dt, rtol, atol, _d(T_out), _d(X_out),
                        _i(nsteps), C.byref(opts), cnt)
     if rc != 0:
         raise ValueError(f"orc_burn failed with code {rc}")
     out = (T_out, X_out, nsteps, dict(zip(COUNTER_NAMES, (int(c) for c in cnt))))
+    if policy:
+        out[3]["nstale"] = int(stale.value)
     if not trace:
         return out
     if int(tn[0]) > int(trace):

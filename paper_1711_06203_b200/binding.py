@@ -11,9 +11,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
 EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_src", "burn_zones_host", "burn_zones_static", "net_destroy",
                     "bz_get_counters",
-                    "bz_norm_lanes", "bz_select_kernel", "bz_kernel_name", "bz_last_cuda_error", "bz_fp64_peak_probe")
+                    "bz_norm_lanes", "bz_select_kernel", "bz_set_schedule", "bz_set_limits", "bz_kernel_name",
+                    "bz_last_cuda_error", "bz_fp64_peak_probe")
 _STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
-           -5: "CUDA runtime error", -6: "out of memory", -7: "unsupported by the forced kernel"}
+           -5: "CUDA runtime error", -6: "out of memory", -7: "unsupported", -8: "handle belongs to another device"}
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -34,8 +35,8 @@ class _Desc(C.Structure):
 
 
 def library_path() -> str:
-    """The in-tree build; BZ_LIBBURN names another build of the same library (kernel experiments)."""
-    return os.environ.get("BZ_LIBBURN") or os.path.join(_HERE, "libburn.so")
+    """The in-tree build (python -m paper_1711_06203_b200.build)."""
+    return os.path.join(_HERE, "libburn.so")
 
 
 _lib = None
@@ -72,6 +73,10 @@ def _L():
         lib.bz_norm_lanes.argtypes = [vp]
         lib.bz_select_kernel.restype = C.c_int
         lib.bz_select_kernel.argtypes = [vp, C.c_int]
+        lib.bz_set_schedule.restype = C.c_int
+        lib.bz_set_schedule.argtypes = [vp, C.c_int]
+        lib.bz_set_limits.restype = C.c_int
+        lib.bz_set_limits.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32]
         lib.bz_kernel_name.restype = C.c_char_p
         lib.bz_kernel_name.argtypes = [vp]
         lib.bz_last_cuda_error.restype = C.c_int
@@ -103,8 +108,16 @@ class Net:
         return _L().bz_kernel_name(self._h).decode()
 
     def select_kernel(self, kind: str = "auto") -> None:
-        """'auto' (specialised quad kernel when available), 'coop' (generic), 'tpz', 'quad'."""
-        _check(_L().bz_select_kernel(self._h, {"auto": 0, "coop": 1, "tpz": 2, "quad": 3}[kind]), "bz_select_kernel")
+        """'auto' (specialised quad kernel when available), 'coop' (generic), 'quad'."""
+        _check(_L().bz_select_kernel(self._h, {"auto": 0, "coop": 1, "quad": 3}[kind]), "bz_select_kernel")
+
+    def set_schedule(self, kind: str = "queue") -> None:
+        """'queue' (work queue, default) or 'static' (round-robin assignment; for measuring a2)."""
+        _check(_L().bz_set_schedule(self._h, {"queue": 0, "static": 1}[kind]), "bz_set_schedule")
+
+    def set_limits(self, mxstep: int = 0, mxnef: int = 0, mxncf: int = 0) -> None:
+        """Limits behind the failure codes -3 / -2 / -1; 0 = default (20000 / 7 / 10)."""
+        _check(_L().bz_set_limits(self._h, int(mxstep), int(mxnef), int(mxncf)), "bz_set_limits")
 
     def close(self):
         if self._h is not None:
@@ -161,12 +174,13 @@ def _stream_ptr(stream):
     return C.c_void_p(s.cuda_stream)
 
 
-def burn_zones(net: Net, rho, T, X, dt, rtol, atol, T_out=None, X_out=None, nsteps=None, stream=None):
-    """Device tensors in, device tensors out (torch, float64, contiguous; X is [nspec, nz]).
-    Enqueues on `stream` (default: torch's current stream) and returns without synchronising."""
+def _device_args(nspec, rho, T, X, extra_in=(), T_out=None, X_out=None, nsteps=None):
+    """Check the device tensors of a burn call (float64 / int32, contiguous, CUDA, right shapes) and
+    create the outputs the caller did not pass.  Marshalling only."""
     import torch
     nz = rho.shape[0]
-    for name, t, shape in (("rho", rho, (nz,)), ("T", T, (nz,)), ("X", X, (net.nspec, nz))):
+    ins = [("rho", rho, (nz,)), ("T", T, (nz,)), ("X", X, (nspec, nz))] + list(extra_in)
+    for name, t, shape in ins:
         if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
             raise ValueError(f"{name} must be a contiguous float64 CUDA tensor of shape {shape}")
     if T_out is None:
@@ -175,13 +189,23 @@ def burn_zones(net: Net, rho, T, X, dt, rtol, atol, T_out=None, X_out=None, nste
         X_out = torch.empty_like(X)
     if nsteps is None:
         nsteps = torch.empty(nz, dtype=torch.int32, device=rho.device)
-    for name, t, dt_, shape in (("T_out", T_out, torch.float64, (nz,)), ("X_out", X_out, torch.float64, (net.nspec, nz)),
+    for name, t, dt_, shape in (("T_out", T_out, torch.float64, (nz,)), ("X_out", X_out, torch.float64, (nspec, nz)),
                                 ("nsteps", nsteps, torch.int32, (nz,))):
         if not (t.is_cuda and t.dtype == dt_ and t.is_contiguous() and tuple(t.shape) == shape):
             raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {shape}")
-    p = lambda t: C.c_void_p(t.data_ptr())
-    _check(_L().burn_zones(net._h, nz, p(rho), p(T), p(X), float(dt), float(rtol), float(atol),
-                           p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones")
+    return nz, T_out, X_out, nsteps
+
+
+def _p(t):
+    return C.c_void_p(t.data_ptr())
+
+
+def burn_zones(net: Net, rho, T, X, dt, rtol, atol, T_out=None, X_out=None, nsteps=None, stream=None):
+    """Device tensors in, device tensors out (torch, float64, contiguous; X is [nspec, nz]).
+    Enqueues on `stream` (default: torch's current stream) and returns without synchronising."""
+    nz, T_out, X_out, nsteps = _device_args(net.nspec, rho, T, X, (), T_out, X_out, nsteps)
+    _check(_L().burn_zones(net._h, nz, _p(rho), _p(T), _p(X), float(dt), float(rtol), float(atol),
+                           _p(T_out), _p(X_out), _p(nsteps), _stream_ptr(stream)), "burn_zones")
     return T_out, X_out, nsteps
 
 
@@ -189,25 +213,11 @@ def burn_zones_src(net: Net, rho, T, X, src_T, src_X, dt, rtol, atol, T_out=None
                    stream=None):
     """burn_zones with constant per-zone source terms (include/burnzones.h: burn_zones_src):
     dT/dt += src_T [nz] (K/s), dX_i/dt += src_X [nspec, nz] (1/s).  Device tensors like burn_zones."""
-    import torch
-    nz = rho.shape[0]
-    for name, t, shape in (("rho", rho, (nz,)), ("T", T, (nz,)), ("X", X, (net.nspec, nz)),
-                           ("src_T", src_T, (nz,)), ("src_X", src_X, (net.nspec, nz))):
-        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
-            raise ValueError(f"{name} must be a contiguous float64 CUDA tensor of shape {shape}")
-    if T_out is None:
-        T_out = torch.empty_like(T)
-    if X_out is None:
-        X_out = torch.empty_like(X)
-    if nsteps is None:
-        nsteps = torch.empty(nz, dtype=torch.int32, device=rho.device)
-    for name, t, dt_, shape in (("T_out", T_out, torch.float64, (nz,)), ("X_out", X_out, torch.float64, (net.nspec, nz)),
-                                ("nsteps", nsteps, torch.int32, (nz,))):
-        if not (t.is_cuda and t.dtype == dt_ and t.is_contiguous() and tuple(t.shape) == shape):
-            raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {shape}")
-    p = lambda t: C.c_void_p(t.data_ptr())
-    _check(_L().burn_zones_src(net._h, nz, p(rho), p(T), p(X), p(src_T), p(src_X), float(dt), float(rtol),
-                               float(atol), p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones_src")
+    nz0 = rho.shape[0]
+    extra = (("src_T", src_T, (nz0,)), ("src_X", src_X, (net.nspec, nz0)))
+    nz, T_out, X_out, nsteps = _device_args(net.nspec, rho, T, X, extra, T_out, X_out, nsteps)
+    _check(_L().burn_zones_src(net._h, nz, _p(rho), _p(T), _p(X), _p(src_T), _p(src_X), float(dt), float(rtol),
+                               float(atol), _p(T_out), _p(X_out), _p(nsteps), _stream_ptr(stream)), "burn_zones_src")
     return T_out, X_out, nsteps
 
 
@@ -224,15 +234,31 @@ def strang_step(net: Net, rho, T, X, dt, rtol, atol, update=None, stream=None):
     return rho, T2, X2, ns1, ns2
 
 
-def burn_zones_host(net: Net, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, stream=None):
-    """Host (ideally pinned) torch tensors or numpy arrays in and out; H2D + burn + D2H are
-    enqueued on `stream`.  The caller synchronises."""
-    nz = rho.shape[0]
+def _host_ptr(name, a, dtype_name, shape):
+    """Address of a host array (numpy, or a CPU torch tensor) after checking dtype, C-contiguity and
+    shape: the library copies exactly prod(shape) elements from/to this address."""
+    if hasattr(a, "data_ptr"):                      # torch tensor
+        if a.is_cuda or str(a.dtype) != f"torch.{dtype_name}" or not a.is_contiguous() or tuple(a.shape) != shape:
+            raise ValueError(f"{name} must be a contiguous CPU {dtype_name} tensor of shape {shape}")
+        return C.c_void_p(a.data_ptr())
+    if not isinstance(a, np.ndarray) or a.dtype != np.dtype(dtype_name) or not a.flags.c_contiguous \
+            or a.shape != shape:
+        raise ValueError(f"{name} must be a C-contiguous {dtype_name} array of shape {shape}")
+    return C.c_void_p(a.ctypes.data)
 
-    def ptr(a):
-        return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
-    _check(_L().burn_zones_host(net._h, nz, ptr(rho), ptr(T), ptr(X), float(dt), float(rtol), float(atol),
-                                ptr(T_out), ptr(X_out), ptr(nsteps), _stream_ptr(stream)), "burn_zones_host")
+
+def burn_zones_host(net: Net, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, stream=None):
+    """Host arrays in and out (numpy or CPU torch tensors; float64, nsteps int32; C-contiguous; X and
+    X_out [nspec, nz]).  H2D + burn + D2H are enqueued on `stream` and the call returns; with PINNED
+    memory it returns without waiting for the copies, with pageable memory the runtime stages each copy
+    before returning.  The caller synchronises the stream before reading the outputs."""
+    nz = rho.shape[0]
+    args = [_host_ptr("rho", rho, "float64", (nz,)), _host_ptr("T", T, "float64", (nz,)),
+            _host_ptr("X", X, "float64", (net.nspec, nz))]
+    outs = [_host_ptr("T_out", T_out, "float64", (nz,)), _host_ptr("X_out", X_out, "float64", (net.nspec, nz)),
+            _host_ptr("nsteps", nsteps, "int32", (nz,))]
+    _check(_L().burn_zones_host(net._h, nz, *args, float(dt), float(rtol), float(atol), *outs, _stream_ptr(stream)),
+           "burn_zones_host")
     return T_out, X_out, nsteps
 
 

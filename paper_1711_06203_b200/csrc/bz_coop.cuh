@@ -45,6 +45,8 @@ struct BurnArgs {
   unsigned long long *queue;     // work-queue head
   unsigned long long *counters;  // [8]
   const double *src_T, *src_X;   // constant source terms (burn_zones_src), both nullptr = none
+  int mxstep, mxnef, mxncf;      // limits behind the failure codes -3 / -2 / -1 (bz_set_limits)
+  int static_sched;              // 1: static round-robin zone assignment instead of the work queue (bz_set_schedule)
 };
 
 __device__ __forceinline__ double inv_small_int(int p) {  // 1.0/p, p = 1..7, correctly rounded

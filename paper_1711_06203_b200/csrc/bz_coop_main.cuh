@@ -67,11 +67,20 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
 #pragma unroll
   for (int i = 0; i <= QMAX; i++) tau[i] = 0.0, Z[i] = 0.0;
 
+  bool started = false;
   for (;;) {
     if (phase == 0) {
       // ---- a2: fetch the next zone from the work queue -------------------------------------------
-      if (lig == 0) z = (long long)atomicAdd(A.queue, 1ull);
-      z = __shfl_sync(g.gmask, z, 0, LANES);
+      // (bz_set_schedule(1) switches a2 off for the before/after measurement: group g then burns zones
+      // g, g + G, g + 2G, ... with G = groups of the grid; results are the same, only the balance differs)
+      if (A.static_sched) {
+        const long long G = (long long)gridDim.x * (COOP_THREADS / LANES);
+        z = started ? z + G : (long long)blockIdx.x * (COOP_THREADS / LANES) + threadIdx.x / LANES;
+        started = true;
+      } else {
+        if (lig == 0) z = (long long)atomicAdd(A.queue, 1ull);
+        z = __shfl_sync(g.gmask, z, 0, LANES);
+      }
       if (z >= A.nz) {
         phase = 2;
       } else {

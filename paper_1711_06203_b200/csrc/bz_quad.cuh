@@ -44,9 +44,9 @@ struct QuadMem {
   // rarely used per-zone scalars, parked here instead of in registers (every lane of the quad
   // stores the same bits and reads them back: no intra-quad synchronisation needed)
   static constexpr int SC_T = 26, SC_ETAMAX = 27, SC_HSAV = 28, SC_ZID = 29, SC_INT = 30, SC_N = 31;
-  static constexpr int CNT_OFF = SC_OFF + SC_N;         // event counters of this quad: 8 x uint32 (lane 0 only)
+  static constexpr int CNT_OFF = SC_OFF + SC_N;         // event counters of this quad: 8 x uint64 (lane 0 only)
   static constexpr int CN_NST = 0, CN_XRHS = 1, CN_INIT = 2, CN_LU = 3, CN_SOL = 4, CN_ETF = 5, CN_CFN = 6, CN_FAIL = 7;
-  static constexpr int SRC_OFF = CNT_OFF + 4;           // constant source terms s[NEQ] (burn_zones_src)
+  static constexpr int SRC_OFF = CNT_OFF + 8;           // constant source terms s[NEQ] (burn_zones_src)
   static constexpr int RAW = SRC_OFF + NEQ;
   static constexpr int SIZE = RAW + ((4 - (RAW % 32) + 32) % 32);  // == 4 (mod 32)
   double *base;
@@ -60,7 +60,7 @@ struct QuadMem {
   __device__ __forceinline__ long long &zid() const { return *reinterpret_cast<long long *>(base + SC_OFF + SC_ZID); }
   __device__ __forceinline__ int &isc(int i) const { return reinterpret_cast<int *>(base + SC_OFF + SC_INT)[i]; }  // 0: qS, 1: ntau
   __device__ __forceinline__ double &src(int i) const { return base[SRC_OFF + i]; }
-  __device__ __forceinline__ unsigned &cnt(int i) const { return reinterpret_cast<unsigned *>(base + CNT_OFF)[i]; }
+  __device__ __forceinline__ unsigned long long &cnt(int i) const { return reinterpret_cast<unsigned long long *>(base + CNT_OFF)[i]; }
 };
 
 // Pascal-triangle predict / retract of one component for a compile-time order Q: no predication,
@@ -173,16 +173,10 @@ struct QuadLU {
       const int ko = k & 3, ks = k >> 2;
       double *ub = m.ub(k & 1);
       if (c == ko) {
-#ifndef BZ_QUAD_ROW_STS128
         volatile double *vb = ub;  // 64-bit stores straight from the row's registers (no tuple packing)
 #pragma unroll
         for (int j = k; j < NEQ; j++) vb[j] = a[ks][j];
         vb[NEQ] = b[ks];
-#else
-#pragma unroll
-        for (int j = k; j < NEQ; j++) ub[j] = a[ks][j];
-        ub[NEQ] = b[ks];
-#endif
       }
       __syncwarp(gmask);
       const double piv = ub[k];

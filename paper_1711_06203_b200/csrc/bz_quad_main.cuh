@@ -38,10 +38,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
   } while (0)
   // event counters live in the quad's shared memory (lane 0 counts): registers are the scarce
   // resource of this kernel.  nrhs = nlu + ninit + xrhs and njac = nlu + ninit are derived at the end.
-#define BZQ_COUNT(k) do { if (c == 0) m.cnt(Mem::k) += 1u; } while (0)
+#define BZQ_COUNT(k) do { if (c == 0) m.cnt(Mem::k) += 1ull; } while (0)
   if (c == 0) {
 #pragma unroll
-    for (int k = 0; k < 8; k++) m.cnt(k) = 0u;
+    for (int k = 0; k < 8; k++) m.cnt(k) = 0ull;
+    m.zid() = gquad - (long long)gridDim.x * (QUAD_THREADS / 4);  // static schedule: first zone = gquad
   }
 
   // component index of my slot s and its validity
@@ -98,8 +99,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
     const bool bulk = __popc(__ballot_sync(0xffffffffu, phase == 0)) >= 8;  // two quads or more
     if (phase == 0) {
       // ---- a2 + a1: next zone, load, validate, initialise ------------------------------------------
+      // (bz_set_schedule(1) switches the queue off for the before/after measurement of a2: quad g then
+      // burns zones g, g + G, g + 2G, ... with G = quads of the grid; same results, different balance)
       long long z = 0;
-      if (c == 0) z = (long long)atomicAdd(A.queue, 1ull);
+      if (c == 0)
+        z = A.static_sched ? m.zid() + (long long)gridDim.x * (QUAD_THREADS / 4) : (long long)atomicAdd(A.queue, 1ull);
       z = __shfl_sync(gmask, z, 0, 4);
       m.zid() = z;
       if (z >= A.nz) {

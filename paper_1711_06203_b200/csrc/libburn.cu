@@ -12,7 +12,6 @@
 
 #include "../../include/burnzones.h"
 #include "bz_coop_main.cuh"
-#include "bz_tpz_main.cuh"
 #include "bz_quad_main.cuh"
 #include "gen/registry.inc"
 
@@ -51,23 +50,7 @@ double host_log(double x) {
 }
 
 typedef void (*KernelFn)(bz::DevNet, bz::BurnArgs);
-typedef void (*TpzKernelFn)(bz::TpzNet, bz::BurnArgs, double *);
-
-// ---- network-specialised thread-per-zone kernels (generated topologies) -----------------------
-constexpr int TPZ_BLOCK = 96, TPZ_W = 4;
-struct TpzVariant {
-  const char *name;
-  unsigned long long topo_hash;
-  int neq, K, smem_bytes;
-  TpzKernelFn fn;
-};
-template <class Net>
-TpzVariant make_tpz(const char *name) {
-  const int tab = (4 * Net::K + Net::N + 1) & ~1;
-  return {name, Net::TOPO_HASH, Net::NEQ, Net::K,
-          (int)sizeof(double) * (tab + bz::TpzMem<Net::NEQ, TPZ_BLOCK>::PER_THREAD * TPZ_BLOCK),
-          (TpzKernelFn)bz::burn_tpz_kernel<Net, TPZ_BLOCK, TPZ_W>};
-}
+// ---- network-specialised 4-lanes-per-zone kernels (generated topologies) ----------
 typedef void (*QuadKernelFn)(bz::QuadNet, bz::BurnArgs);
 struct QuadVariant {
   const char *name;
@@ -82,16 +65,10 @@ QuadVariant make_quad(const char *name) {
           (int)sizeof(double) * (tab + bz::QuadMem<Net::NEQ, Net::K>::SIZE * (BLOCK / 4)), BLOCK,
           (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB>};
 }
-// two block shapes with the same register budget (<= 168): 3 blocks of 128 threads per SM, or one
-// block of 384 threads per SM (all 12 warps share one barrier per trip = one instruction stream;
-// measured 1.8x faster, profiles/README.md).  BZ_QUAD_SHAPE=128x3|384x1 picks one at net_create.
-#define BZ_QUAD_ENTRY3(NET) make_quad<NET, 128, 3>("burn_quad<" #NET ",128x3>"),
-#define BZ_QUAD_ENTRY2(NET) make_quad<NET, 384, 1>("burn_quad<" #NET ",384x1>"),
-const QuadVariant kQuad3[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY3)};
-const QuadVariant kQuad2[] = {BZ_TPZ_NETS(BZ_QUAD_ENTRY2)};
-
-#define BZ_TPZ_ENTRY(NET) make_tpz<NET>("burn_tpz<" #NET ">"),
-const TpzVariant kTpz[] = {BZ_TPZ_NETS(BZ_TPZ_ENTRY)};
+// one block of 384 threads per SM (<= 168 registers): all 12 warps share one barrier per trip = one
+// instruction stream (3 blocks of 128 threads were 1.8x slower, profiles/README.md)
+#define BZ_QUAD_ENTRY(NET) make_quad<NET, 384, 1>("burn_quad<" #NET ",384x1>"),
+const QuadVariant kQuad[] = {BZ_GEN_NETS(BZ_QUAD_ENTRY)};
 
 // FNV-1a over the topology; must equal paper_1711_06203_b200/codegen.py:topology_hash
 unsigned long long topology_hash(const bz_net_desc *d) {
@@ -143,344 +120,6 @@ const Variant *pick_variant(int n) {
 }
 
 }  // namespace
-
-struct bz_net {
-  int N, n, K;
-  bz::DevNet dev;
-  double *d_dbl;
-  int *d_int;
-  unsigned long long *d_scratch;  // [0] queue head, [1..8] counters
-  const Variant *variant;
-  int grid, smem_bytes;
-  const TpzVariant *tpz;  // non-null: a specialised kernel exists for this topology
-  int tpz_grid;
-  double *d_tpz_coef, *d_tpz_S;
-  const QuadVariant *quad;
-  int quad_grid;
-  double *d_quad_scratch;
-  double fac;
-  int kind;  // 0 auto, 1 cooperative, 2 thread-per-zone, 3 quad
-  // staging for burn_zones_host
-  double *st_in, *st_out;
-  int32_t *st_nsteps;
-  int64_t st_cap;
-};
-
-extern "C" {
-
-int bz_last_cuda_error(void) { return g_last_cuda_error; }
-
-int net_create(const bz_net_desc *d, bz_net **out) {
-  if (!d || !out) return BZ_ERR_NULL;
-  *out = nullptr;
-  if (d->nspec < 1 || d->nspec > 31 || d->nreac < 1 || d->nreac > 256) return BZ_ERR_SIZE;
-  if (!d->aion || !d->reactant || !d->stoich_id || !d->stoich_dy || !d->rate_A || !d->rate_n ||
-      !d->rate_B || !d->q_mev)
-    return BZ_ERR_NULL;
-  const int N = d->nspec, K = d->nreac, n = N + 1;
-  if (!(d->cv > 0.0) || !std::isfinite(d->cv)) return BZ_ERR_NETWORK;
-  for (int i = 0; i < N; i++)
-    if (!(d->aion[i] > 0.0) || !std::isfinite(d->aion[i])) return BZ_ERR_NETWORK;
-
-  // ---- flatten -------------------------------------------------------------------------------
-  std::vector<int> rp(4 * K, 0);
-  std::vector<double> lnA(K), invsym(K);
-  std::vector<std::vector<std::pair<int, double>>> sp(N);  // species -> (k, dy), k ascending
-  std::vector<std::vector<int>> cl(N);                     // species -> (k | slot << 16)
-  for (int k = 0; k < K; k++) {
-    int r[3], m = 0;
-    for (int a = 0; a < 3; a++) {
-      const int id = d->reactant[3 * k + a];
-      if (id < 0) continue;
-      if (id >= N) return BZ_ERR_NETWORK;
-      r[m++] = id;
-    }
-    if (m == 0) return BZ_ERR_NETWORK;
-    if (!(d->rate_A[k] > 0.0) || !std::isfinite(d->rate_A[k]) || !std::isfinite(d->rate_n[k]) ||
-        !std::isfinite(d->rate_B[k]) || !std::isfinite(d->q_mev[k]))
-      return BZ_ERR_NETWORK;
-    // distinct reactant species in order of first appearance = Jacobian column slots
-    int col[3] = {0, 0, 0}, nslot = 0;
-    for (int a = 0; a < m; a++) {
-      bool seen = false;
-      for (int b = 0; b < a; b++) seen |= (r[b] == r[a]);
-      if (!seen) col[nslot++] = r[a];
-    }
-    const int same = (m > 1 && r[0] == r[1]) + (m > 2 && r[0] == r[2]) + (m > 2 && r[1] == r[2]);
-    invsym[k] = same == 0 ? 1.0 : (same == 1 ? 0.5 : 1.0 / 6.0);
-    lnA[k] = host_log(d->rate_A[k]);
-    rp[4 * k + 0] = m | (nslot << 8);
-    rp[4 * k + 1] = r[0] | ((m > 1 ? r[1] : 0) << 8) | ((m > 2 ? r[2] : 0) << 16);
-    rp[4 * k + 2] = col[0] | (col[1] << 8) | (col[2] << 16);
-    for (int s = 0; s < nslot; s++) cl[col[s]].push_back(k | (s << 16));
-    int ids[4], nid = 0;
-    for (int a = 0; a < 4; a++) {
-      const int id = d->stoich_id[4 * k + a];
-      if (id < 0) continue;
-      if (id >= N) return BZ_ERR_NETWORK;
-      for (int b = 0; b < nid; b++)
-        if (ids[b] == id) return BZ_ERR_NETWORK;
-      if (!std::isfinite(d->stoich_dy[4 * k + a])) return BZ_ERR_NETWORK;
-      ids[nid++] = id;
-      sp[id].push_back({k, d->stoich_dy[4 * k + a]});
-    }
-  }
-  std::vector<int> sp_off(N + 1, 0), sp_k, cl_off(N + 1, 0), cl_ks;
-  std::vector<double> sp_dy;
-  for (int i = 0; i < N; i++) {
-    for (auto &t : sp[i]) {
-      sp_k.push_back(t.first);
-      sp_dy.push_back(t.second);
-    }
-    sp_off[i + 1] = (int)sp_k.size();
-    for (int c : cl[i]) cl_ks.push_back(c);
-    cl_off[i + 1] = (int)cl_ks.size();
-  }
-  const int nterm = (int)sp_k.size(), ncl = (int)cl_ks.size();
-  std::vector<double> dbl;
-  dbl.insert(dbl.end(), lnA.begin(), lnA.end());
-  dbl.insert(dbl.end(), d->rate_n, d->rate_n + K);
-  dbl.insert(dbl.end(), d->rate_B, d->rate_B + K);
-  dbl.insert(dbl.end(), d->q_mev, d->q_mev + K);
-  dbl.insert(dbl.end(), invsym.begin(), invsym.end());
-  dbl.insert(dbl.end(), d->aion, d->aion + N);
-  dbl.insert(dbl.end(), sp_dy.begin(), sp_dy.end());
-  std::vector<int> itab;
-  itab.insert(itab.end(), rp.begin(), rp.end());
-  itab.insert(itab.end(), sp_off.begin(), sp_off.end());
-  itab.insert(itab.end(), sp_k.begin(), sp_k.end());
-  itab.insert(itab.end(), cl_off.begin(), cl_off.end());
-  itab.insert(itab.end(), cl_ks.begin(), cl_ks.end());
-
-  bz_net *h = new (std::nothrow) bz_net();
-  if (!h) return BZ_ERR_NOMEM;
-  std::memset(h, 0, sizeof(*h));
-  h->N = N; h->n = n; h->K = K;
-  h->variant = pick_variant(n);
-
-  // ---- upload --------------------------------------------------------------------------------
-  auto fail = [&](int code) {
-    net_destroy(h);
-    return code;
-  };
-  if (!cuda_ok(cudaMalloc(&h->d_dbl, dbl.size() * sizeof(double)))) return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaMalloc(&h->d_int, itab.size() * sizeof(int)))) return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaMalloc(&h->d_scratch, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaMemcpy(h->d_dbl, dbl.data(), dbl.size() * sizeof(double), cudaMemcpyHostToDevice)))
-    return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaMemcpy(h->d_int, itab.data(), itab.size() * sizeof(int), cudaMemcpyHostToDevice)))
-    return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaMemset(h->d_scratch, 0, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
-  h->dev.N = N; h->dev.n = n; h->dev.K = K; h->dev.nterm = nterm; h->dev.ncl = ncl;
-  h->dev.fac = 9.648533212331e17 / d->cv;
-  h->dev.dbl = h->d_dbl; h->dev.itab = h->d_int;
-  h->dev.ndbl = (int)dbl.size(); h->dev.nint = (int)itab.size();
-
-  // ---- launch geometry: persistent grid, blocks/SM from the occupancy calculator -----------------
-  const int L = h->variant->lanes;
-  const int gpb = bz::COOP_THREADS / L;
-  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
-  const int tab = ((h->dev.ndbl + 1) & ~1) + (((h->dev.nint + 3) & ~3) / 2);
-  h->smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
-  int dev = 0, sms = 0, bps = 0;
-  if (!cuda_ok(cudaGetDevice(&dev))) return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev))) return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaFuncSetAttribute((const void *)h->variant->fn,
-                                    cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes)))
-    return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->variant->fn,
-                                                             bz::COOP_THREADS, h->smem_bytes)))
-    return fail(BZ_ERR_CUDA);
-  if (bps < 1) return fail(BZ_ERR_NOMEM);
-  h->grid = sms * bps;
-  h->fac = h->dev.fac;
-
-  // ---- specialised thread-per-zone kernel for known topologies ------------------------------------
-  const unsigned long long th = topology_hash(d);
-  for (const TpzVariant &v : kTpz)
-    if (v.topo_hash == th && v.neq == n && v.K == K) h->tpz = &v;
-  if (h->tpz) {
-    std::vector<double> tc;
-    tc.insert(tc.end(), lnA.begin(), lnA.end());
-    tc.insert(tc.end(), d->rate_n, d->rate_n + K);
-    tc.insert(tc.end(), d->rate_B, d->rate_B + K);
-    tc.insert(tc.end(), d->q_mev, d->q_mev + K);
-    tc.insert(tc.end(), d->aion, d->aion + N);
-    if (!cuda_ok(cudaMalloc(&h->d_tpz_coef, tc.size() * sizeof(double)))) return fail(BZ_ERR_CUDA);
-    if (!cuda_ok(cudaMemcpy(h->d_tpz_coef, tc.data(), tc.size() * sizeof(double), cudaMemcpyHostToDevice)))
-      return fail(BZ_ERR_CUDA);
-    int tb = 0;
-    if (!cuda_ok(cudaFuncSetAttribute((const void *)h->tpz->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      h->tpz->smem_bytes)))
-      return fail(BZ_ERR_CUDA);
-    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&tb, (const void *)h->tpz->fn, TPZ_BLOCK,
-                                                               h->tpz->smem_bytes)))
-      return fail(BZ_ERR_CUDA);
-    if (tb < 1) return fail(BZ_ERR_NOMEM);
-    h->tpz_grid = sms * tb;
-    if (!cuda_ok(cudaMalloc(&h->d_tpz_S, (size_t)n * h->tpz_grid * TPZ_BLOCK * sizeof(double))))
-      return fail(BZ_ERR_CUDA);
-    const QuadVariant *tab = kQuad2;  // default: 384x1
-    if (const char *e = std::getenv("BZ_QUAD_SHAPE")) {
-      if (!std::strcmp(e, "128x3")) tab = kQuad3;
-    }
-    const int ntab = (int)(sizeof(kQuad3) / sizeof(kQuad3[0]));
-    for (int i = 0; i < ntab; i++)
-      if (tab[i].topo_hash == th && tab[i].neq == n && tab[i].K == K) h->quad = &tab[i];
-  }
-  if (h->quad) {
-    int qb = 0;
-    if (!cuda_ok(cudaFuncSetAttribute((const void *)h->quad->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      h->quad->smem_bytes)))
-      return fail(BZ_ERR_CUDA);
-    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&qb, (const void *)h->quad->fn, h->quad->block,
-                                                               h->quad->smem_bytes)))
-      return fail(BZ_ERR_CUDA);
-    if (qb < 1) return fail(BZ_ERR_NOMEM);
-    h->quad_grid = sms * qb;
-    const size_t per_quad = (size_t)n * n + 2 * n;
-    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * h->quad_grid * (h->quad->block / 4) * sizeof(double))))
-      return fail(BZ_ERR_CUDA);
-  }
-  *out = h;
-  return BZ_OK;
-}
-
-int net_destroy(bz_net *h) {
-  if (!h) return BZ_ERR_NULL;
-  if (h->d_dbl) cudaFree(h->d_dbl);
-  if (h->d_int) cudaFree(h->d_int);
-  if (h->d_scratch) cudaFree(h->d_scratch);
-  if (h->d_tpz_coef) cudaFree(h->d_tpz_coef);
-  if (h->d_tpz_S) cudaFree(h->d_tpz_S);
-  if (h->d_quad_scratch) cudaFree(h->d_quad_scratch);
-  if (h->st_in) cudaFree(h->st_in);
-  if (h->st_out) cudaFree(h->st_out);
-  if (h->st_nsteps) cudaFree(h->st_nsteps);
-  delete h;
-  return BZ_OK;
-}
-
-static bool use_quad(const bz_net *h) { return h->quad && (h->kind == 0 || h->kind == 3); }
-static bool use_tpz(const bz_net *h) { return h->tpz && h->kind == 2; }
-int bz_norm_lanes(const bz_net *h) {
-  return h ? ((use_quad(h) || use_tpz(h)) ? 4 : h->variant->lanes) : BZ_ERR_NULL;
-}
-const char *bz_kernel_name(const bz_net *h) {
-  return h ? (use_quad(h) ? h->quad->name : (use_tpz(h) ? h->tpz->name : h->variant->name)) : "";
-}
-int bz_select_kernel(bz_net *h, int kind) {
-  if (!h) return BZ_ERR_NULL;
-  if (kind < 0 || kind > 3) return BZ_ERR_SIZE;
-  h->kind = kind;
-  return BZ_OK;
-}
-
-int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
-               double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
-               void *cuda_stream) {
-  return burn_zones_src(h, nz, rho, T, X, nullptr, nullptr, dt, rtol, atol, T_out, X_out, nsteps, cuda_stream);
-}
-
-int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
-                   const double *src_T, const double *src_X, double dt, double rtol, double atol,
-                   double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream) {
-  if (!h) return BZ_ERR_NULL;
-  if (nz < 0) return BZ_ERR_SIZE;
-  if (!(dt > 0.0) || !(rtol > 0.0) || !(atol >= 0.0) || !std::isfinite(dt) || !std::isfinite(rtol) ||
-      !std::isfinite(atol))
-    return BZ_ERR_SCALAR;
-  if (nz == 0) return BZ_OK;
-  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
-  if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
-  if (src_T && !use_quad(h) && use_tpz(h)) return BZ_ERR_UNSUPPORTED;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  BZ_CUDA(cudaMemsetAsync(h->d_scratch, 0, 16 * sizeof(unsigned long long), st));
-  bz::BurnArgs a;
-  a.src_T = src_T; a.src_X = src_X;
-  a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
-  a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
-  a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
-  if (use_quad(h)) {
-    bz::QuadNet qn;
-    qn.coef = h->d_tpz_coef;
-    qn.fac = h->fac;
-    qn.gscratch = h->d_quad_scratch;
-    const int zpb = h->quad->block / 4;
-    const long long blocks_needed = (nz + zpb - 1) / zpb;
-    const int grid = (int)(blocks_needed < h->quad_grid ? blocks_needed : h->quad_grid);
-    void *qargs[] = {(void *)&qn, (void *)&a};
-    BZ_CUDA(cudaLaunchKernel((const void *)h->quad->fn, dim3(grid), dim3(h->quad->block), qargs,
-                             (size_t)h->quad->smem_bytes, st));
-    return BZ_OK;
-  }
-  if (use_tpz(h)) {
-    bz::TpzNet tn;
-    tn.coef = h->d_tpz_coef;
-    tn.fac = h->fac;
-    const long long blocks_needed = (nz + TPZ_BLOCK - 1) / TPZ_BLOCK;
-    const int grid = (int)(blocks_needed < h->tpz_grid ? blocks_needed : h->tpz_grid);
-    double *S = h->d_tpz_S;
-    void *targs[] = {(void *)&tn, (void *)&a, (void *)&S};
-    BZ_CUDA(cudaLaunchKernel((const void *)h->tpz->fn, dim3(grid), dim3(TPZ_BLOCK), targs,
-                             (size_t)h->tpz->smem_bytes, st));
-    return BZ_OK;
-  }
-  const int L = h->variant->lanes;
-  const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
-  const int grid = (int)(groups_needed < h->grid ? groups_needed : h->grid);
-  void *args[] = {(void *)&h->dev, (void *)&a};
-  BZ_CUDA(cudaLaunchKernel((const void *)h->variant->fn, dim3(grid), dim3(bz::COOP_THREADS), args,
-                           (size_t)h->smem_bytes, st));
-  return BZ_OK;
-}
-
-int bz_get_counters(const bz_net *h, void *cuda_stream, uint64_t out[8]) {
-  if (!h || !out) return BZ_ERR_NULL;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  unsigned long long tmp[8];
-  BZ_CUDA(cudaMemcpyAsync(tmp, h->d_scratch + 1, sizeof(tmp), cudaMemcpyDeviceToHost, st));
-  BZ_CUDA(cudaStreamSynchronize(st));
-  for (int i = 0; i < 8; i++) out[i] = tmp[i];
-  return BZ_OK;
-}
-
-int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
-                    double dt, double rtol, double atol, double *T_out, double *X_out,
-                    int32_t *nsteps, void *cuda_stream) {
-  if (!h) return BZ_ERR_NULL;
-  if (nz < 0) return BZ_ERR_SIZE;
-  if (nz == 0) return BZ_OK;
-  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int N = h->N;
-  if (h->st_cap < nz) {
-    BZ_CUDA(cudaStreamSynchronize(st));
-    if (h->st_in) cudaFree(h->st_in);
-    if (h->st_out) cudaFree(h->st_out);
-    if (h->st_nsteps) cudaFree(h->st_nsteps);
-    h->st_in = h->st_out = nullptr;
-    h->st_nsteps = nullptr;
-    h->st_cap = 0;
-    if (!cuda_ok(cudaMalloc(&h->st_in, (size_t)(N + 2) * nz * sizeof(double)))) return BZ_ERR_NOMEM;
-    if (!cuda_ok(cudaMalloc(&h->st_out, (size_t)(N + 1) * nz * sizeof(double)))) return BZ_ERR_NOMEM;
-    if (!cuda_ok(cudaMalloc(&h->st_nsteps, (size_t)nz * sizeof(int32_t)))) return BZ_ERR_NOMEM;
-    h->st_cap = nz;
-  }
-  double *d_rho = h->st_in, *d_T = h->st_in + nz, *d_X = h->st_in + 2 * nz;
-  double *d_To = h->st_out, *d_Xo = h->st_out + nz;
-  BZ_CUDA(cudaMemcpyAsync(d_rho, rho, nz * sizeof(double), cudaMemcpyHostToDevice, st));
-  BZ_CUDA(cudaMemcpyAsync(d_T, T, nz * sizeof(double), cudaMemcpyHostToDevice, st));
-  BZ_CUDA(cudaMemcpyAsync(d_X, X, (size_t)N * nz * sizeof(double), cudaMemcpyHostToDevice, st));
-  int rc = burn_zones(h, nz, d_rho, d_T, d_X, dt, rtol, atol, d_To, d_Xo, h->st_nsteps, cuda_stream);
-  if (rc != BZ_OK) return rc;
-  BZ_CUDA(cudaMemcpyAsync(T_out, d_To, nz * sizeof(double), cudaMemcpyDeviceToHost, st));
-  BZ_CUDA(cudaMemcpyAsync(X_out, d_Xo, (size_t)N * nz * sizeof(double), cudaMemcpyDeviceToHost, st));
-  BZ_CUDA(cudaMemcpyAsync(nsteps, h->st_nsteps, nz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-  return BZ_OK;
-}
-
-}  // extern "C"
 
 // ---- burn_zones_static: the burn without any device allocation ------------------------------------
 // Everything the cooperative kernel needs besides the caller's arrays -- work-queue head, counters,
@@ -611,6 +250,275 @@ int static_flatten(const bz_net_desc *d, StaticFlat &F) {
 }
 }  // namespace
 
+
+struct bz_net {
+  int N, n, K;
+  bz::DevNet dev;
+  double *d_dbl;
+  int *d_int;
+  unsigned long long *d_scratch;  // [0] queue head, [1..8] counters
+  const Variant *variant;
+  int grid, smem_bytes;
+  const QuadVariant *quad;  // non-null: a specialised kernel exists for this topology
+  int quad_grid;
+  double *d_quad_coef, *d_quad_scratch;
+  double fac;
+  int kind;        // 0 auto, 1 cooperative, 3 quad (bz_select_kernel)
+  int device;      // the device that was current at net_create: a handle belongs to ONE device
+  int static_sched;  // bz_set_schedule: 0 = work queue (a2), 1 = static round-robin assignment
+  int mxstep, mxnef, mxncf;  // bz_set_limits
+  // staging for burn_zones_host
+  double *st_in, *st_out;
+  int32_t *st_nsteps;
+  int64_t st_cap;
+};
+
+extern "C" {
+
+int bz_last_cuda_error(void) { return g_last_cuda_error; }
+
+int net_create(const bz_net_desc *d, bz_net **out) {
+  if (!d || !out) return BZ_ERR_NULL;
+  *out = nullptr;
+  if (d->nspec < 1 || d->nspec > 31 || d->nreac < 1 || d->nreac > 256) return BZ_ERR_SIZE;
+  if (!d->aion || !d->reactant || !d->stoich_id || !d->stoich_dy || !d->rate_A || !d->rate_n ||
+      !d->rate_B || !d->q_mev)
+    return BZ_ERR_NULL;
+  const int N = d->nspec, K = d->nreac, n = N + 1;
+  // ---- validate + flatten (host only: bad descriptors are refused before CUDA is touched) ---------
+  static thread_local StaticFlat F;
+  const int frc = static_flatten(d, F);
+  if (frc != BZ_OK) return frc;
+
+  bz_net *h = new (std::nothrow) bz_net();
+  if (!h) return BZ_ERR_NOMEM;
+  std::memset(h, 0, sizeof(*h));
+  h->N = N; h->n = n; h->K = K;
+  h->variant = pick_variant(n);
+  h->mxstep = bz::MXSTEP; h->mxnef = bz::MXNEF; h->mxncf = bz::MXNCF;
+
+  // ---- upload --------------------------------------------------------------------------------
+  auto fail = [&](int code) {
+    net_destroy(h);
+    return code;
+  };
+  if (!cuda_ok(cudaGetDevice(&h->device))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMalloc(&h->d_dbl, F.ndbl * sizeof(double)))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMalloc(&h->d_int, F.nint * sizeof(int)))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMalloc(&h->d_scratch, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMemcpy(h->d_dbl, F.dbl, F.ndbl * sizeof(double), cudaMemcpyHostToDevice)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMemcpy(h->d_int, F.itab, F.nint * sizeof(int), cudaMemcpyHostToDevice)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaMemset(h->d_scratch, 0, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
+  h->dev.N = N; h->dev.n = n; h->dev.K = K; h->dev.nterm = F.nterm; h->dev.ncl = F.ncl;
+  h->dev.fac = 9.648533212331e17 / d->cv;
+  h->dev.dbl = h->d_dbl; h->dev.itab = h->d_int;
+  h->dev.ndbl = F.ndbl; h->dev.nint = F.nint;
+  h->fac = h->dev.fac;
+
+  // ---- launch geometry: persistent grid, blocks/SM from the occupancy calculator -----------------
+  const int L = h->variant->lanes;
+  const int gpb = bz::COOP_THREADS / L;
+  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
+  const int tab = ((h->dev.ndbl + 1) & ~1) + (((h->dev.nint + 3) & ~3) / 2);
+  h->smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
+  int sms = 0, bps = 0, optin = 0;
+  if (!cuda_ok(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device))) return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device)))
+    return fail(BZ_ERR_CUDA);
+  if (h->smem_bytes > optin) return fail(BZ_ERR_NOMEM);
+  // the attribute belongs to the kernel, not to the handle: always opt in to the device maximum, so
+  // that a later handle with smaller tables cannot lower it under an earlier one
+  if (!cuda_ok(cudaFuncSetAttribute((const void *)h->variant->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->variant->fn,
+                                                             bz::COOP_THREADS, h->smem_bytes)))
+    return fail(BZ_ERR_CUDA);
+  if (bps < 1) return fail(BZ_ERR_NOMEM);
+  h->grid = sms * bps;
+
+  // ---- network-specialised quad kernel for known topologies ---------------------------------------
+  const unsigned long long th = topology_hash(d);
+  for (const QuadVariant &v : kQuad)
+    if (v.topo_hash == th && v.neq == n && v.K == K) h->quad = &v;
+  if (h->quad) {
+    // coefficient table of the generated code: lnA[K] n[K] B[K] Q[K] aion[N]
+    double qc[4 * ST_MAXK + ST_MAXN];
+    for (int k = 0; k < K; k++) {
+      qc[k] = F.dbl[k]; qc[K + k] = d->rate_n[k]; qc[2 * K + k] = d->rate_B[k]; qc[3 * K + k] = d->q_mev[k];
+    }
+    for (int i = 0; i < N; i++) qc[4 * K + i] = d->aion[i];
+    if (!cuda_ok(cudaMalloc(&h->d_quad_coef, (4 * K + N) * sizeof(double)))) return fail(BZ_ERR_CUDA);
+    if (!cuda_ok(cudaMemcpy(h->d_quad_coef, qc, (4 * K + N) * sizeof(double), cudaMemcpyHostToDevice)))
+      return fail(BZ_ERR_CUDA);
+    int qb = 0;
+    if (h->quad->smem_bytes > optin) return fail(BZ_ERR_NOMEM);
+    if (!cuda_ok(cudaFuncSetAttribute((const void *)h->quad->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
+      return fail(BZ_ERR_CUDA);
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&qb, (const void *)h->quad->fn, h->quad->block,
+                                                               h->quad->smem_bytes)))
+      return fail(BZ_ERR_CUDA);
+    if (qb < 1) return fail(BZ_ERR_NOMEM);
+    h->quad_grid = sms * qb;
+    const size_t per_quad = (size_t)n * n + 2 * n;
+    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * h->quad_grid * (h->quad->block / 4) * sizeof(double))))
+      return fail(BZ_ERR_CUDA);
+  }
+  *out = h;
+  return BZ_OK;
+}
+
+int net_destroy(bz_net *h) {
+  if (!h) return BZ_ERR_NULL;
+  if (h->d_dbl) cudaFree(h->d_dbl);
+  if (h->d_int) cudaFree(h->d_int);
+  if (h->d_scratch) cudaFree(h->d_scratch);
+  if (h->d_quad_coef) cudaFree(h->d_quad_coef);
+  if (h->d_quad_scratch) cudaFree(h->d_quad_scratch);
+  if (h->st_in) cudaFree(h->st_in);
+  if (h->st_out) cudaFree(h->st_out);
+  if (h->st_nsteps) cudaFree(h->st_nsteps);
+  delete h;
+  return BZ_OK;
+}
+
+static bool use_quad(const bz_net *h) { return h->quad && (h->kind == 0 || h->kind == 3); }
+int bz_norm_lanes(const bz_net *h) { return h ? (use_quad(h) ? 4 : h->variant->lanes) : BZ_ERR_NULL; }
+const char *bz_kernel_name(const bz_net *h) { return h ? (use_quad(h) ? h->quad->name : h->variant->name) : ""; }
+int bz_select_kernel(bz_net *h, int kind) {
+  if (!h) return BZ_ERR_NULL;
+  if (kind != 0 && kind != 1 && kind != 3) return BZ_ERR_SIZE;
+  h->kind = kind;
+  return BZ_OK;
+}
+int bz_set_schedule(bz_net *h, int kind) {
+  if (!h) return BZ_ERR_NULL;
+  if (kind != 0 && kind != 1) return BZ_ERR_SIZE;
+  h->static_sched = kind;
+  return BZ_OK;
+}
+int bz_set_limits(bz_net *h, int32_t mxstep, int32_t mxnef, int32_t mxncf) {
+  if (!h) return BZ_ERR_NULL;
+  if (mxstep < 0 || mxnef < 0 || mxncf < 0) return BZ_ERR_SIZE;
+  h->mxstep = mxstep > 0 ? mxstep : bz::MXSTEP;
+  h->mxnef = mxnef > 0 ? mxnef : bz::MXNEF;
+  h->mxncf = mxncf > 0 ? mxncf : bz::MXNCF;
+  return BZ_OK;
+}
+
+// a handle's tables, scratch, grid size and shared-memory opt-in belong to the device that was
+// current at net_create: a call made with another device current is refused, not misexecuted
+static int check_device(const bz_net *h) {
+  int dev = -1;
+  BZ_CUDA(cudaGetDevice(&dev));
+  return dev == h->device ? BZ_OK : BZ_ERR_DEVICE;
+}
+
+int burn_zones(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+               double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
+               void *cuda_stream) {
+  return burn_zones_src(h, nz, rho, T, X, nullptr, nullptr, dt, rtol, atol, T_out, X_out, nsteps, cuda_stream);
+}
+
+static bool scalars_ok(double dt, double rtol, double atol) {
+  return (dt > 0.0) && (rtol > 0.0) && (atol >= 0.0) && std::isfinite(dt) && std::isfinite(rtol) && std::isfinite(atol);
+}
+
+int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+                   const double *src_T, const double *src_X, double dt, double rtol, double atol,
+                   double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream) {
+  if (!h) return BZ_ERR_NULL;
+  if (nz < 0) return BZ_ERR_SIZE;
+  if (!scalars_ok(dt, rtol, atol)) return BZ_ERR_SCALAR;
+  if (nz == 0) return BZ_OK;
+  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
+  const int drc = check_device(h);
+  if (drc != BZ_OK) return drc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  BZ_CUDA(cudaMemsetAsync(h->d_scratch, 0, 16 * sizeof(unsigned long long), st));
+  bz::BurnArgs a;
+  a.src_T = src_T; a.src_X = src_X;
+  a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
+  a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
+  a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
+  a.mxstep = h->mxstep; a.mxnef = h->mxnef; a.mxncf = h->mxncf;
+  a.static_sched = h->static_sched;
+  if (use_quad(h)) {
+    bz::QuadNet qn;
+    qn.coef = h->d_quad_coef;
+    qn.fac = h->fac;
+    qn.gscratch = h->d_quad_scratch;
+    const int zpb = h->quad->block / 4;
+    const long long blocks_needed = (nz + zpb - 1) / zpb;
+    const int grid = (int)(blocks_needed < h->quad_grid ? blocks_needed : h->quad_grid);
+    void *qargs[] = {(void *)&qn, (void *)&a};
+    BZ_CUDA(cudaLaunchKernel((const void *)h->quad->fn, dim3(grid), dim3(h->quad->block), qargs,
+                             (size_t)h->quad->smem_bytes, st));
+    return BZ_OK;
+  }
+  const int L = h->variant->lanes;
+  const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
+  const int grid = (int)(groups_needed < h->grid ? groups_needed : h->grid);
+  void *args[] = {(void *)&h->dev, (void *)&a};
+  BZ_CUDA(cudaLaunchKernel((const void *)h->variant->fn, dim3(grid), dim3(bz::COOP_THREADS), args,
+                           (size_t)h->smem_bytes, st));
+  return BZ_OK;
+}
+
+int bz_get_counters(const bz_net *h, void *cuda_stream, uint64_t out[8]) {
+  if (!h || !out) return BZ_ERR_NULL;
+  const int drc = check_device(h);
+  if (drc != BZ_OK) return drc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned long long tmp[8];
+  BZ_CUDA(cudaMemcpyAsync(tmp, h->d_scratch + 1, sizeof(tmp), cudaMemcpyDeviceToHost, st));
+  BZ_CUDA(cudaStreamSynchronize(st));
+  for (int i = 0; i < 8; i++) out[i] = tmp[i];
+  return BZ_OK;
+}
+
+int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+                    double dt, double rtol, double atol, double *T_out, double *X_out,
+                    int32_t *nsteps, void *cuda_stream) {
+  if (!h) return BZ_ERR_NULL;
+  if (nz < 0) return BZ_ERR_SIZE;
+  if (!scalars_ok(dt, rtol, atol)) return BZ_ERR_SCALAR;  // before anything is staged or enqueued
+  if (nz == 0) return BZ_OK;
+  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  const int drc = check_device(h);
+  if (drc != BZ_OK) return drc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int N = h->N;
+  if (h->st_cap < nz) {
+    BZ_CUDA(cudaStreamSynchronize(st));
+    if (h->st_in) cudaFree(h->st_in);
+    if (h->st_out) cudaFree(h->st_out);
+    if (h->st_nsteps) cudaFree(h->st_nsteps);
+    h->st_in = h->st_out = nullptr;
+    h->st_nsteps = nullptr;
+    h->st_cap = 0;
+    if (!cuda_ok(cudaMalloc(&h->st_in, (size_t)(N + 2) * nz * sizeof(double)))) return BZ_ERR_NOMEM;
+    if (!cuda_ok(cudaMalloc(&h->st_out, (size_t)(N + 1) * nz * sizeof(double)))) return BZ_ERR_NOMEM;
+    if (!cuda_ok(cudaMalloc(&h->st_nsteps, (size_t)nz * sizeof(int32_t)))) return BZ_ERR_NOMEM;
+    h->st_cap = nz;
+  }
+  double *d_rho = h->st_in, *d_T = h->st_in + nz, *d_X = h->st_in + 2 * nz;
+  double *d_To = h->st_out, *d_Xo = h->st_out + nz;
+  BZ_CUDA(cudaMemcpyAsync(d_rho, rho, nz * sizeof(double), cudaMemcpyHostToDevice, st));
+  BZ_CUDA(cudaMemcpyAsync(d_T, T, nz * sizeof(double), cudaMemcpyHostToDevice, st));
+  BZ_CUDA(cudaMemcpyAsync(d_X, X, (size_t)N * nz * sizeof(double), cudaMemcpyHostToDevice, st));
+  int rc = burn_zones(h, nz, d_rho, d_T, d_X, dt, rtol, atol, d_To, d_Xo, h->st_nsteps, cuda_stream);
+  if (rc != BZ_OK) return rc;
+  BZ_CUDA(cudaMemcpyAsync(T_out, d_To, nz * sizeof(double), cudaMemcpyDeviceToHost, st));
+  BZ_CUDA(cudaMemcpyAsync(X_out, d_Xo, (size_t)N * nz * sizeof(double), cudaMemcpyDeviceToHost, st));
+  BZ_CUDA(cudaMemcpyAsync(nsteps, h->st_nsteps, nz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  return BZ_OK;
+}
+
+}  // extern "C"
+
 extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double *rho, const double *T,
                                  const double *X, double dt, double rtol, double atol, double *T_out,
                                  double *X_out, int32_t *nsteps, void *cuda_stream) {
@@ -669,6 +577,8 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = reinterpret_cast<unsigned long long *>(base);
   a.counters = reinterpret_cast<unsigned long long *>(base) + 1;
+  a.mxstep = bz::MXSTEP; a.mxnef = bz::MXNEF; a.mxncf = bz::MXNCF;
+  a.static_sched = 0;
   const long long groups_needed = (nz + gpb - 1) / gpb;
   const long long full = (long long)sd->sms * bps;
   const int grid = (int)(groups_needed < full ? groups_needed : full);
@@ -706,21 +616,24 @@ extern "C" int bz_fp64_peak_probe(int64_t iters, void *cuda_stream, double *tflo
   BZ_CUDA(cudaGetDevice(&dev));
   BZ_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   double *sink = nullptr;
-  BZ_CUDA(cudaMalloc(&sink, sizeof(double)));
-  cudaEvent_t e0, e1;
-  BZ_CUDA(cudaEventCreate(&e0));
-  BZ_CUDA(cudaEventCreate(&e1));
-  const int blocks = sms * 8, threads = 256;
-  dfma_probe_kernel<<<blocks, threads, 0, st>>>(iters / 8 + 1, sink);  // warm-up
-  BZ_CUDA(cudaEventRecord(e0, st));
-  dfma_probe_kernel<<<blocks, threads, 0, st>>>(iters, sink);
-  BZ_CUDA(cudaEventRecord(e1, st));
-  BZ_CUDA(cudaEventSynchronize(e1));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
   float t = 0.f;
-  BZ_CUDA(cudaEventElapsedTime(&t, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(sink);
+  const int blocks = sms * 8, threads = 256;
+  bool ok = cuda_ok(cudaMalloc(&sink, sizeof(double)));
+  ok = ok && cuda_ok(cudaEventCreate(&e0)) && cuda_ok(cudaEventCreate(&e1));
+  if (ok) {
+    dfma_probe_kernel<<<blocks, threads, 0, st>>>(iters / 8 + 1, sink);  // warm-up
+    ok = cuda_ok(cudaEventRecord(e0, st));
+  }
+  if (ok) {
+    dfma_probe_kernel<<<blocks, threads, 0, st>>>(iters, sink);
+    ok = cuda_ok(cudaEventRecord(e1, st)) && cuda_ok(cudaEventSynchronize(e1)) &&
+         cuda_ok(cudaEventElapsedTime(&t, e0, e1));
+  }
+  if (e0) cudaEventDestroy(e0);  // released on every path
+  if (e1) cudaEventDestroy(e1);
+  if (sink) cudaFree(sink);
+  if (!ok) return BZ_ERR_CUDA;
   const double flops = 2.0 * 8.0 * 32.0 * (double)iters * (double)blocks * (double)threads;
   *ms = (double)t;
   *tflops = flops / ((double)t * 1e-3) / 1e12;

@@ -1,0 +1,150 @@
+"""GPU twins of the oracle pins of tests/test_oracle_nordsieck.py (VERDICT round 1, next-round items 1
+and 2): the SAME inputs that drive the oracle through its rarely taken branches -- the order-1
+restart and the order reduction after a third error-test failure (C.2-B.5), the failure codes -1,
+-2, -3 -- go through every kernel and must come back bit-identical; one test per config compares the
+kernel with the oracle's PLAIN norm definition (norm_lanes = 1) at north_star's tolerance; and the
+work queue can be switched off without changing a bit."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload, network_for_config
+from _parity import compare, X_FLOOR, X_RTOL, T_RTOL
+from test_oracle_nordsieck import _zero_fuel_source_zones, _stress_zones
+
+pytestmark = pytest.mark.gpu
+OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+def _record(tag, stats):
+    os.makedirs(OUT, exist_ok=True)
+    with open(os.path.join(OUT, "parity_stats.jsonl"), "a") as fh:
+        fh.write(json.dumps(dict(tag=tag, **stats)) + "\n")
+
+
+def _burn(net_d, rho, T, X, dt, rtol, atol, kind, src=None, limits=None, schedule="queue"):
+    import torch
+    import paper_1711_06203_b200 as bz
+    dev = torch.device("cuda:0")
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    net = bz.net_create(net_d)
+    net.select_kernel(kind)
+    net.set_schedule(schedule)
+    if limits:
+        net.set_limits(**limits)
+    if src is None:
+        To, Xo, ns = bz.burn_zones(net, d(rho), d(T), d(X), dt, rtol, atol)
+    else:
+        To, Xo, ns = bz.burn_zones_src(net, d(rho), d(T), d(X), d(src[0]), d(src[1]), dt, rtol, atol)
+    torch.cuda.synchronize()
+    out = To.cpu().numpy(), Xo.cpu().numpy(), ns.cpu().numpy(), bz.get_counters(net), net.norm_lanes, net.kernel_name
+    bz.net_destroy(net)
+    return out
+
+
+def _same(gpu, ref):
+    To, Xo, ns, cnt = gpu[:4]
+    Tr, Xr, nr, cr = ref
+    assert np.array_equal(ns, nr)
+    assert np.array_equal(To, Tr) and np.array_equal(Xo, Xr)
+    assert all(cnt[k] == cr[k] for k in cnt), (cnt, cr)
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["auto", "coop"])
+def test_order1_restart_on_gpu(kind):
+    """C.2-B.5 at q = 1 (third error-test failure: h <- 0.1 h, Z_1 = h f): reached by real inputs --
+    config 1's network with no fuel and a carbon source (tests/test_oracle_nordsieck.py)."""
+    net_d, rho, T, X, sT, sX = _zero_fuel_source_zones(1500)
+    gpu = _burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, kind, src=(sT, sX))
+    oracle.event_counts(reset=True)
+    ref = oracle.burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, norm_lanes=gpu[4], src_T=sT, src_X=sX)
+    ev = oracle.event_counts()
+    assert ev["etf_restart_order1"] > 100, ev
+    _same(gpu, ref)
+    _record(f"restart:{kind}", dict(kernel=gpu[5], **ev))
+
+
+@pytest.mark.parametrize("kind", ["auto", "coop"])
+def test_failure_code_minus1_on_gpu(kind):
+    """atol = 0 with exactly zero abundances: infinite weights, every Newton norm non-finite, eleven
+    quarterings, code -1; then with the limit lowered to 3 failures."""
+    w = make_workload(3, zones=2039)
+    for limits, nfail in ((None, 11), (dict(mxncf=3), 4)):
+        gpu = _burn(w.net, w.rho, w.T, w.X, w.dt, 1e-8, 0.0, kind, limits=limits)
+        ref = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, 1e-8, 0.0, norm_lanes=gpu[4], **(limits or {}))
+        assert (ref[2] == -1).all() and ref[3]["ncfn"] == nfail * w.nz
+        _same(gpu, ref)
+
+
+@pytest.mark.parametrize("kind", ["auto", "coop"])
+def test_failure_codes_minus2_minus3_through_the_limits(kind):
+    """-2: the inputs whose third error-test failure is real (the restart zones) with mxnef = 3;
+    -3: config 3 zones with a budget of 100 steps.  Same limits on both sides, bit-identical."""
+    net_d, rho, T, X, sT, sX = _zero_fuel_source_zones(1500)
+    lim = dict(mxnef=3)
+    gpu = _burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, kind, src=(sT, sX), limits=lim)
+    ref = oracle.burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, norm_lanes=gpu[4], src_T=sT, src_X=sX, **lim)
+    assert (ref[2] == -2).sum() > 100 and (ref[2] > 0).sum() > 100
+    _same(gpu, ref)
+    w = make_workload(3, zones=2039)
+    lim = dict(mxstep=100)
+    gpu = _burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, kind, limits=lim)
+    ref = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=gpu[4], **lim)
+    assert (ref[2] == -3).sum() > 100 and (ref[2] > 0).sum() > 10
+    _same(gpu, ref)
+    _record(f"limits:{kind}", dict(kernel=gpu[5], n_minus3=int((ref[2] == -3).sum())))
+
+
+@pytest.mark.parametrize("kind", ["auto", "coop"])
+def test_order_reduction_zones_on_gpu(kind):
+    """The four stress zones on which the oracle's B.5 order reduction was checked against the exact
+    interpolant (test_order_reduction_after_third_failure_keeps_the_interpolant), with neighbours."""
+    for trial, zones in ((2, (789, 840)), (3, (955, 973))):
+        net_d, rho, T, X, dt = _stress_zones(trial)
+        idx = np.unique(np.concatenate([np.arange(z - 8, z + 8) for z in zones]))
+        r, t, x = rho[idx], T[idx], np.ascontiguousarray(X[:, idx])
+        gpu = _burn(net_d, r, t, x, dt, 1e-8, 1e-12, kind)
+        oracle.event_counts(reset=True)
+        ref = oracle.burn(net_d, r, t, x, dt, 1e-8, 1e-12, norm_lanes=gpu[4])
+        assert oracle.event_counts()["etf_lower_order"] >= 2
+        _same(gpu, ref)
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,zones", [(1, None), (2, 127), (3, 1021), (4, None), (5, 8191)])
+def test_against_the_plain_norm_definition(config, zones):
+    """The kernel's norm association (4 / 32 interleaved partial sums) is a declared parameter that the
+    bit-exact tests hand to the oracle.  Here the oracle uses its PLAIN definition (one sequential sum,
+    norm_lanes = 1): the two trajectories then differ by rounding in the norms, and the result must
+    still meet north_star's bar: 1e-5 on X > 1e-10, 1e-6 on T.  Records the worst ratio to the bound."""
+    if config == 4:
+        w0 = make_workload(4, zones=[0])
+        c = w0.meta["centres"][:8].astype(int)
+        lines = [np.arange(256) + 256 * (cc[1] + 256 * cc[2]) for cc in c]      # x-lines through 8 hotspots
+        zones = np.unique(np.concatenate(lines + [np.arange(0, 256 ** 3, 65521)]))
+    w = make_workload(config, zones=zones)
+    gpu = _burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, "auto")
+    Tr, Xr, nr, _ = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=1)
+    stats = compare(gpu[0], gpu[1], gpu[2], Tr, Xr, nr)          # asserts the bar
+    stats.update(kernel=gpu[5], worst_X_ratio_to_bound=stats["max_rel_X"] / X_RTOL,
+                 worst_T_ratio_to_bound=stats["max_rel_T"] / T_RTOL)
+    _record(f"plain_norm:config{config}", stats)
+    assert stats["nz"] >= 1000
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["auto", "coop"])
+def test_static_schedule_gives_the_same_bits(kind):
+    """bz_set_schedule(1) replaces the work queue (step a2) by a static round-robin assignment: every
+    zone is still burned exactly once and the results do not change."""
+    c = make_workload(4, zones=[0]).meta["centres"][0].astype(int)
+    slab = (np.arange(256)[None, :] + 256 * (np.arange(c[1] - 8, c[1] + 8)[:, None] + 256 * c[2])).ravel()
+    w = make_workload(4, zones=np.sort(slab))
+    a = _burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, kind, schedule="queue")
+    b = _burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, kind, schedule="static")
+    assert a[2].min() == 1 and a[2].max() > 100
+    _same(b, (a[0], a[1], a[2], a[3]))

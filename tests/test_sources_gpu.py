@@ -85,7 +85,7 @@ def test_closed_form_with_source_on_gpu():
     assert abs(Xo[0, 0] / 4 - YP) <= 100 * (1e-8 * YP + 1e-12)
 
 
-def test_invalid_and_unsupported_sources():
+def test_invalid_sources():
     import torch
     import paper_1711_06203_b200 as bz
     w = make_workload(1, zones=[1, 2, 3, 4])
@@ -103,12 +103,6 @@ def test_invalid_and_unsupported_sources():
         assert ns[0] > 0 and ns[3] > 0 and ns[1] == -4 and ns[2] == -4, (kind, ns)
         assert np.array_equal(To.cpu().numpy()[1:3], w.T[1:3]) and np.array_equal(Xo.cpu().numpy()[:, 1:3], w.X[:, 1:3])
         bz.net_destroy(net)
-    net = bz.net_create(w.net)
-    net.select_kernel("tpz")          # the thread-per-zone kernel has no source path: the call says so
-    with pytest.raises(bz.BurnError) as e:
-        bz.burn_zones_src(net, d(w.rho), d(w.T), d(w.X), d(np.zeros(4)), d(sX * 0), w.dt, w.rtol, w.atol)
-    assert e.value.code == -7
-    bz.net_destroy(net)
 
 
 def test_strang_step_matches_two_oracle_half_burns():
