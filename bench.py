@@ -168,6 +168,7 @@ def run_ours(args):
     net = bz.net_create(w.net)
     net.select_kernel(args.kernel)
     net.set_schedule("static" if args.static_schedule else "queue")
+    net.set_policy(args.policy)
     stream = torch.cuda.current_stream()
 
     # ---- device-resident arm -------------------------------------------------------------------
@@ -247,7 +248,7 @@ def run_ours(args):
         tpath = os.path.join(ROOT, "profiles", "ncu_counters.json")
         if os.path.exists(tpath):
             rec = json.load(open(tpath)).get(f"config{cfg}:{net.kernel_name}")
-            if rec and not args.static_schedule:
+            if rec and not args.static_schedule and args.policy == "fresh":
                 traffic, executed, ncu_src = rec.get("dram_bytes"), rec.get("executed_fp64_flops"), rec.get("source")
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -257,6 +258,8 @@ def run_ours(args):
                        "zones_per_gpu": nz, "neq": N + 1, "nreac": w.net.nreac,
                        "dt": w.dt, "rtol": w.rtol, "atol": w.atol, "kernel": net.kernel_name,
                        "schedule": "static round-robin (a2 off)" if args.static_schedule else "work queue (a2)",
+                       "newton_matrix": "fresh J + LU every attempt (BZ-BDF v1)" if args.policy == "fresh"
+                                        else "reused, VODE-style (BZ-BDF v2, DESIGN.md 12)",
                        "l2": (f"inputs {8 * (N + 2) * nz / 1e6:.0f} MB per step exceed the 126 MB L2" if 8 * (N + 2) * nz > 126e6
                               else f"inputs {8 * (N + 2) * nz / 1e6:.1f} MB per step fit the L2; the kernel is ALU-bound, "
                                    "state traffic is < 1e-3 of its time"),
@@ -282,17 +285,18 @@ def run_ours(args):
         }
         if not args.no_cpu_baseline and world == 1:
             import oracle
+            pol = 1 if args.policy == "reuse" else 0
             stride = CPU_SAMPLE_STRIDE[cfg]
             ws = make_workload(cfg, zones=stride if stride > 1 else None)
             t0 = time.perf_counter()
-            oracle.burn(ws.net, ws.rho, ws.T, ws.X, ws.dt, ws.rtol, ws.atol)
+            oracle.burn(ws.net, ws.rho, ws.T, ws.X, ws.dt, ws.rtol, ws.atol, policy=pol)
             el = time.perf_counter() - t0
             out["cpu_baseline"] = {"value": ws.nz / el, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
                                    "sample": f"every {stride}th zone ({ws.nz} zones), {el:.1f} s wall"}
             s1 = SINGLE_CORE_STRIDE[cfg]
             w1 = make_workload(cfg, zones=s1 if s1 > 1 else None)
             t0 = time.perf_counter()
-            oracle.burn(w1.net, w1.rho, w1.T, w1.X, w1.dt, w1.rtol, w1.atol, nthreads=1)
+            oracle.burn(w1.net, w1.rho, w1.T, w1.X, w1.dt, w1.rtol, w1.atol, nthreads=1, policy=pol)
             el1 = time.perf_counter() - t0
             out["cpu_baseline"]["single_core"] = {"value": w1.nz / el1, "unit": UNIT, "cores": 1,
                                                   "sample": f"every {s1}th zone ({w1.nz} zones), {el1:.1f} s wall"}
@@ -329,6 +333,8 @@ def main():
                     help="auto = specialised quad kernel when the topology has one, else the generic coop kernel")
     ap.add_argument("--static-schedule", action="store_true",
                     help="switch the work queue (step a2) off: static round-robin zone assignment, for the before/after figure")
+    ap.add_argument("--policy", default="fresh", choices=["fresh", "reuse"],
+                    help="Newton matrix: fresh J + LU on every attempt (default, the parity reference) or VODE-style reuse")
     ap.add_argument("--stride", type=int, default=1,
                     help="burn every S-th zone of the config only (short ncu captures; not a bench value)")
     ap.add_argument("--stub", action="store_true", help=argparse.SUPPRESS)   # tests only: see run_stub

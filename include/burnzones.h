@@ -41,7 +41,8 @@ typedef enum {
   BZ_ERR_SCALAR = -4,  /* dt <= 0, rtol <= 0, atol < 0, or non-finite                         */
   BZ_ERR_CUDA = -5,    /* CUDA runtime error; the cudaError_t is in bz_last_cuda_error()      */
   BZ_ERR_NOMEM = -6,   /* host or device allocation failed                                    */
-  BZ_ERR_UNSUPPORTED = -7, /* reserved (was: the forced kernel cannot do what was asked)           */
+  BZ_ERR_UNSUPPORTED = -7, /* the selected kernel cannot do what was asked (bz_set_policy 1 on the
+                              generic cooperative kernel)                                          */
   BZ_ERR_DEVICE = -8   /* the handle was created on another device than the current one        */
 } bz_status;
 
@@ -61,6 +62,12 @@ typedef struct {
   const double *rate_A, *rate_n, *rate_B; /* [K]                                              */
   const double *q_mev;       /* [K]    Q-values, MeV per reaction event                        */
   double cv;                 /* specific heat, erg g^-1 K^-1, constant                         */
+  const double *rate_rho_exp; /* [K] or NULL: optional density exponents e_k of weak rates -- lambda_k
+                                is multiplied by rho^e_k ON TOP of the rho^(m_k - 1) of the rate law
+                                (electron captures grow with density, beta decays are blocked by it:
+                                "the 9-isotope Urca network").  Evaluated
+                                inside the exponent: arg_k += e_k * ln(rho).  Finite values; NULL = none.
+                                Networks that carry it run on the generic cooperative kernel.            */
 } bz_net_desc;
 
 /* Validate, flatten and upload a network.  *out receives the handle.  A handle belongs to the
@@ -158,6 +165,22 @@ int bz_select_kernel(bz_net *net, int kind);
  * kind 1 = static round-robin assignment (group g burns zones g, g + G, g + 2G, ...), kept only so
  * that the benefit of the queue can be MEASURED (bench.py --static-schedule).  Results are identical. */
 int bz_set_schedule(bz_net *net, int kind);
+
+/* Newton-matrix policy ("we ported our workhorse ODE integrator (VODE [33])",
+ * PAPER.md:L119, and VODE reuses its factorised Newton matrix, ref. [33] L184).
+ *   kind 0 (default, "BZ-BDF v1", the parity reference of BASELINE.json): a fresh Jacobian and LU on
+ *          every step attempt.
+ *   kind 1 ("BZ-BDF v2"): the LU of P = I - gamma_P J is kept; an attempt evaluates J
+ *          and factorises only if there is no matrix yet, |gamma/gamma_P - 1| > 0.3, 20 steps were
+ *          accepted since, or a failure asked for it; corrections solved with the kept matrix are
+ *          scaled by 2/(1 + gamma/gamma_P); a Newton failure with a kept matrix repeats the attempt at
+ *          the same step size with a fresh one.  About 12x fewer factorisations on the alpha-chain
+ *          configs at the same step count.  Results are bit-identical to the oracle's policy 1 (not
+ *          to policy 0: the two differ at the level of the integration tolerance).  Validated on the
+ *          smooth networks (configs 1-4); on config 5 it loses accuracy on trace species.
+ * Served by the network-specialised kernels only: with kind 1, burn_zones on a network that runs on
+ * the generic cooperative kernel returns BZ_ERR_UNSUPPORTED. */
+int bz_set_policy(bz_net *net, int kind);
 
 /* Limits behind the per-zone failure codes: accepted steps (-3), error-test failures on one step
  * (-2), Newton failures on one step (-1).  0 keeps the default (20000, 7, 10); negative: BZ_ERR_SIZE.

@@ -97,6 +97,8 @@ typedef struct {
   int sid[ORC_KMAX][4];
   double sdy[ORC_KMAX][4];
   double lnA[ORC_KMAX], en[ORC_KMAX], B[ORC_KMAX], Q[ORC_KMAX], invsym[ORC_KMAX];
+  int has_rexp;            /* the descriptor carries density exponents */
+  double rexp[ORC_KMAX];
   double fac;              /* N_A MeV / c_v                          */
 } Net;
 
@@ -107,6 +109,7 @@ static int net_init(Net *nt, const orc_net_desc *d) {
   nt->K = d->nreac;
   if (!(d->cv > 0.0)) return -3;
   nt->fac = NA_MEV / d->cv;
+  nt->has_rexp = (d->rate_rho_exp != NULL);
   for (int i = 0; i < nt->N; i++) {
     if (!(d->aion[i] > 0.0)) return -3;
     nt->aion[i] = d->aion[i];
@@ -138,6 +141,11 @@ static int net_init(Net *nt, const orc_net_desc *d) {
     nt->en[k] = d->rate_n[k];
     nt->B[k] = d->rate_B[k];
     nt->Q[k] = d->q_mev[k];
+    nt->rexp[k] = 0.0;
+    if (d->rate_rho_exp) {
+      if (!isfinite(d->rate_rho_exp[k])) return -3;
+      nt->rexp[k] = d->rate_rho_exp[k];
+    }
     /* 1 / prod_i nu_ik!  (reading s2): 1, 1/2 (one pair), 1/6 (triple) */
     int r0 = nt->r[k][0], r1 = m > 1 ? nt->r[k][1] : -1, r2 = m > 2 ? nt->r[k][2] : -2;
     int same = (r0 == r1) + (r0 == r2) + (r1 == r2);
@@ -179,10 +187,13 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
   const double t13third = t13 * (1.0 / 3.0);
   const double invT = 1.0 / T;
   const double rhopow[4] = {0.0, 1.0, rho, rho * rho};
+  /* density exponents (optional): lambda_k *= rho^e_k, taken into the exponent with the own log */
+  const double lnrho = nt->has_rexp ? orc_log(rho) : 0.0;
   for (int k = 0; k < nt->K; k++) {
     const int m = nt->m[k];
     const int *r = nt->r[k];
     double arg = fma(-nt->B[k], t13, fma(nt->en[k], lnT9, nt->lnA[k]));
+    if (nt->has_rexp) arg = fma(nt->rexp[k], lnrho, arg);
     double lam = orc_exp(arg);
     double pref = (lam * rhopow[m]) * nt->invsym[k];
     int anyneg = 0;

@@ -49,6 +49,10 @@ typedef struct {
   const double *rate_A, *rate_n, *rate_B; /* [K] lambda = A T9^n exp(-B T9^(-1/3))       */
   const double *q_mev;       /* [K]    MeV per event                                     */
   double cv;                 /* erg/g/K                                                  */
+  /* optional density exponents (weak rates that depend on rho, "the 9-isotope Urca
+   * network"): lambda_k is multiplied by rho^rate_rho_exp[k] ON TOP of the rho^(m-1) of
+   * the rate law, evaluated inside the exponent: arg_k += rate_rho_exp[k] * ln(rho).  NULL = none. */
+  const double *rate_rho_exp; /* [K] or NULL */
 } orc_net_desc;
 
 typedef struct {

@@ -16,7 +16,7 @@ _ip = C.POINTER(C.c_int32)
 class _Desc(C.Structure):
     _fields_ = [("nspec", C.c_int32), ("nreac", C.c_int32), ("aion", _dp), ("reactant", _ip),
                 ("stoich_id", _ip), ("stoich_dy", _dp), ("rate_A", _dp), ("rate_n", _dp),
-                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double)]
+                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double), ("rate_rho_exp", _dp)]
 
 
 class _Opts(C.Structure):
@@ -88,9 +88,14 @@ def _desc(net):
         rate_B=np.ascontiguousarray(net.rate_B, dtype=np.float64),
         q_mev=np.ascontiguousarray(net.q_mev, dtype=np.float64),
     )
+    rexp = getattr(net, "rate_rho_exp", None)
+    if rexp is not None:
+        keep["rate_rho_exp"] = np.ascontiguousarray(rexp, dtype=np.float64)
+        assert keep["rate_rho_exp"].shape == keep["rate_A"].shape
     d = _Desc(int(keep["aion"].shape[0]), int(keep["rate_A"].shape[0]), _d(keep["aion"]),
               _i(keep["reactant"]), _i(keep["stoich_id"]), _d(keep["stoich_dy"]), _d(keep["rate_A"]),
-              _d(keep["rate_n"]), _d(keep["rate_B"]), _d(keep["q_mev"]), float(net.cv))
+              _d(keep["rate_n"]), _d(keep["rate_B"]), _d(keep["q_mev"]), float(net.cv),
+              _d(keep["rate_rho_exp"]) if rexp is not None else None)
     return d, keep
 
 

@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
 EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_src", "burn_zones_host", "burn_zones_static", "net_destroy",
                     "bz_get_counters",
-                    "bz_norm_lanes", "bz_select_kernel", "bz_set_schedule", "bz_set_limits", "bz_kernel_name",
+                    "bz_norm_lanes", "bz_select_kernel", "bz_set_schedule", "bz_set_limits", "bz_set_policy", "bz_kernel_name",
                     "bz_last_cuda_error", "bz_fp64_peak_probe")
 _STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
            -5: "CUDA runtime error", -6: "out of memory", -7: "unsupported", -8: "handle belongs to another device"}
@@ -31,7 +31,7 @@ class BurnError(RuntimeError):
 class _Desc(C.Structure):
     _fields_ = [("nspec", C.c_int32), ("nreac", C.c_int32), ("aion", _dp), ("reactant", _ip),
                 ("stoich_id", _ip), ("stoich_dy", _dp), ("rate_A", _dp), ("rate_n", _dp),
-                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double)]
+                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double), ("rate_rho_exp", _dp)]
 
 
 def library_path() -> str:
@@ -75,6 +75,8 @@ def _L():
         lib.bz_select_kernel.argtypes = [vp, C.c_int]
         lib.bz_set_schedule.restype = C.c_int
         lib.bz_set_schedule.argtypes = [vp, C.c_int]
+        lib.bz_set_policy.restype = C.c_int
+        lib.bz_set_policy.argtypes = [vp, C.c_int]
         lib.bz_set_limits.restype = C.c_int
         lib.bz_set_limits.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32]
         lib.bz_kernel_name.restype = C.c_char_p
@@ -115,6 +117,11 @@ class Net:
         """'queue' (work queue, default) or 'static' (round-robin assignment; for measuring a2)."""
         _check(_L().bz_set_schedule(self._h, {"queue": 0, "static": 1}[kind]), "bz_set_schedule")
 
+    def set_policy(self, kind: str = "fresh") -> None:
+        """'fresh' (Jacobian + LU on every attempt, default) or 'reuse' (VODE-style kept Newton matrix;
+        specialised kernels only)."""
+        _check(_L().bz_set_policy(self._h, {"fresh": 0, "reuse": 1}[kind]), "bz_set_policy")
+
     def set_limits(self, mxstep: int = 0, mxnef: int = 0, mxncf: int = 0) -> None:
         """Limits behind the failure codes -3 / -2 / -1; 0 = default (20000 / 7 / 10)."""
         _check(_L().bz_set_limits(self._h, int(mxstep), int(mxnef), int(mxncf)), "bz_set_limits")
@@ -140,7 +147,7 @@ def _i32(a):
 
 
 def net_create(net=None, *, aion=None, reactant=None, stoich_id=None, stoich_dy=None, rate_A=None,
-               rate_n=None, rate_B=None, q_mev=None, cv=None) -> Net:
+               rate_n=None, rate_B=None, q_mev=None, cv=None, rate_rho_exp=None) -> Net:
     """net_create(rates, Q-values, isotope masses): `net` is any object with those fields
     (e.g. workloads.Network), or pass them as keywords."""
     g = (lambda k, v: v if v is not None else getattr(net, k))
@@ -154,14 +161,25 @@ def net_create(net=None, *, aion=None, reactant=None, stoich_id=None, stoich_dy=
     for k in ("rate_n", "rate_B", "q_mev"):
         if keep[k].shape != (K,):
             raise ValueError(f"{k} must be [K]")
+    rexp = rate_rho_exp if rate_rho_exp is not None else getattr(net, "rate_rho_exp", None)
     d = _Desc(N, K, keep["aion"].ctypes.data_as(_dp), keep["reactant"].ctypes.data_as(_ip),
               keep["stoich_id"].ctypes.data_as(_ip), keep["stoich_dy"].ctypes.data_as(_dp),
               keep["rate_A"].ctypes.data_as(_dp), keep["rate_n"].ctypes.data_as(_dp),
               keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp),
-              float(g("cv", cv)))
+              float(g("cv", cv)), _rexp_ptr(rexp, K, keep))
     h = C.c_void_p()
     _check(_L().net_create(C.byref(d), C.byref(h)), "net_create")
     return Net(h, N, K)
+
+
+def _rexp_ptr(rexp, K, keep):
+    """Optional density exponents [K] -> pointer (NULL when absent); the array is kept alive in `keep`."""
+    if rexp is None:
+        return None
+    keep["rate_rho_exp"] = _f64(rexp)
+    if keep["rate_rho_exp"].shape != (K,):
+        raise ValueError("rate_rho_exp must be [K]")
+    return keep["rate_rho_exp"].ctypes.data_as(_dp)
 
 
 def net_destroy(net: Net) -> None:
@@ -290,7 +308,8 @@ def burn_zones_static(desc, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, str
     d = _Desc(N, K, keep["aion"].ctypes.data_as(_dp), keep["reactant"].ctypes.data_as(_ip),
               keep["stoich_id"].ctypes.data_as(_ip), keep["stoich_dy"].ctypes.data_as(_dp),
               keep["rate_A"].ctypes.data_as(_dp), keep["rate_n"].ctypes.data_as(_dp),
-              keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp), float(desc.cv))
+              keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp), float(desc.cv),
+              _rexp_ptr(getattr(desc, "rate_rho_exp", None), K, keep))
     p = lambda t: C.c_void_p(t.data_ptr())
     _check(_L().burn_zones_static(C.byref(d), nz, p(rho), p(T), p(X), float(dt), float(rtol), float(atol),
                                   p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones_static")

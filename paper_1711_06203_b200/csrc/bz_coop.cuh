@@ -26,14 +26,19 @@ constexpr int QMAX = 5, MAXCOR = 3, MXNCF = 10, MXNEF = 7, MXSTEP = 20000;
 constexpr double NTOL = 0.1, CRDOWN = 0.3, RDIV = 2.0, ETACF = 0.25;
 constexpr double BIAS1 = 4.0, BIAS2 = 6.0, BIAS3 = 10.0, ADDON = 1e-6, THRESH = 1.5;
 constexpr double ETAMIN = 0.1, ETAMXF = 0.2, ETAMX1 = 1e4, ETAMAX = 2.0, SLIVER = 1e-6;
+// Newton-matrix reuse (bz_set_policy 1, "BZ-BDF v2"): refactor when |gamma/gamma_P - 1|
+// exceeds CCMAX or MSBP steps were accepted since the last factorisation
+constexpr double CCMAX = 0.3;
+constexpr int MSBP = 20;
 
 // flat network tables in device memory (built by net_create)
 struct DevNet {
   int N, n, K, nterm, ncl;
   double fac;             // N_A MeV / cv
-  const double *dbl;      // lnA[K] en[K] B[K] Q[K] invsym[K] aion[N] sp_dy[nterm]
+  const double *dbl;      // lnA[K] en[K] B[K] Q[K] invsym[K] aion[N] sp_dy[nterm] (+ rexp[K] if has_rexp)
   const int *itab;        // rp[4K] sp_off[N+1] sp_k[nterm] cl_off[N+1] cl_ks[ncl]
   int ndbl, nint;
+  int has_rexp;           // density exponents of weak rates present (bz_net_desc.rate_rho_exp)
 };
 
 struct BurnArgs {

@@ -8,10 +8,14 @@
 
 namespace bz {
 
-constexpr int COOP_THREADS = 256;  // one block per SM (<= 255 registers per thread)
-
+constexpr int COOP_THREADS = 256;
+// Blocks per SM: the warp-per-zone instances (LANES == 32: a row of up to 32 doubles per lane) need the
+// full 255 registers, one block per SM; with 128 registers they spill 1.7 KB per thread and ran 28 %
+// slower.  The sub-warp instances fit 128 registers, and two blocks per SM (16 warps instead of 8) ran
+// 9 % faster (config 3 on burn_coop<14,16>) -- when shared memory allows two blocks, which net_create
+// asks the occupancy calculator.
 template <int NEQ, int LANES>
-__global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, BurnArgs A) {
+__global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop_kernel(DevNet net, BurnArgs A) {
   extern __shared__ __align__(16) double smem[];
   constexpr int LD = LANES + 1;
   const int N = net.N, n = net.n, K = net.K;
@@ -30,6 +34,7 @@ __global__ void __launch_bounds__(COOP_THREADS) burn_coop_kernel(DevNet net, Bur
   g.inv_n = 1.0 / (double)n;
   g.lnA = s_dbl; g.en = s_dbl + K; g.B = s_dbl + 2 * K; g.Q = s_dbl + 3 * K; g.invsym = s_dbl + 4 * K;
   g.aion = s_dbl + 5 * K; g.sp_dy = s_dbl + 5 * K + N;
+  g.rexp = net.has_rexp ? s_dbl + 5 * K + N + net.nterm : nullptr;
   g.rp = s_int; g.sp_off = s_int + 4 * K; g.sp_k = g.sp_off + (N + 1);
   g.cl_off = g.sp_k + net.nterm; g.cl_ks = g.cl_off + (N + 1);
   {

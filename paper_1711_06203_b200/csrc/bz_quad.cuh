@@ -43,7 +43,11 @@ struct QuadMem {
   static constexpr int SC_L = 0, SC_HS = 7, SC_RXI = 13, SC_TAU = 19;
   // rarely used per-zone scalars, parked here instead of in registers (every lane of the quad
   // stores the same bits and reads them back: no intra-quad synchronisation needed)
-  static constexpr int SC_T = 26, SC_ETAMAX = 27, SC_HSAV = 28, SC_ZID = 29, SC_INT = 30, SC_N = 31;
+  static constexpr int SC_T = 26, SC_ETAMAX = 27, SC_HSAV = 28, SC_ZID = 29, SC_INT = 30;
+  // Newton-matrix reuse (bz_set_policy 1): gamma_P of the kept factorisation; two ints: flags (bit 0 a
+  // factorisation exists, bit 1 a failure asked for a fresh one, bit 2 it lives on the general path)
+  // and nst at the factorisation
+  static constexpr int SC_GAMP = 31, SC_PINT = 32, SC_N = 33;
   static constexpr int CNT_OFF = SC_OFF + SC_N;         // event counters of this quad: 8 x uint64 (lane 0 only)
   static constexpr int CN_NST = 0, CN_XRHS = 1, CN_INIT = 2, CN_LU = 3, CN_SOL = 4, CN_ETF = 5, CN_CFN = 6, CN_FAIL = 7;
   static constexpr int SRC_OFF = CNT_OFF + 8;           // constant source terms s[NEQ] (burn_zones_src)
@@ -59,6 +63,7 @@ struct QuadMem {
   __device__ __forceinline__ double &sc(int i) const { return base[SC_OFF + i]; }
   __device__ __forceinline__ long long &zid() const { return *reinterpret_cast<long long *>(base + SC_OFF + SC_ZID); }
   __device__ __forceinline__ int &isc(int i) const { return reinterpret_cast<int *>(base + SC_OFF + SC_INT)[i]; }  // 0: qS, 1: ntau
+  __device__ __forceinline__ int &pint(int i) const { return reinterpret_cast<int *>(base + SC_OFF + SC_PINT)[i]; }  // 0: flags, 1: nslp
   __device__ __forceinline__ double &src(int i) const { return base[SRC_OFF + i]; }
   __device__ __forceinline__ unsigned long long &cnt(int i) const { return reinterpret_cast<unsigned long long *>(base + CNT_OFF)[i]; }
 };
@@ -164,8 +169,10 @@ struct QuadLU {
   // general path often enough to cost 18 % of that config.)
   // b: right-hand side of the first solve; its forward elimination (dgesl, k ascending) rides along:
   // the pivot row's b_k is published with the row, so the first solve needs only back_solve().
+  // wf (quad-uniform): this quad factorises.  With wf false (Newton-matrix reuse: the quad keeps its
+  // factors) the quad goes through the same instruction stream but changes neither a nor b.
   template <class Mem>
-  __device__ __forceinline__ unsigned factor(const Mem &m, int c, unsigned gmask, double (&b)[S]) {
+  __device__ __forceinline__ unsigned factor(const Mem &m, int c, unsigned gmask, double (&b)[S], const bool wf) {
     unsigned lmax = 0u;
     bool bad = false;
 #pragma unroll
@@ -183,11 +190,11 @@ struct QuadLU {
       const double bk = ub[NEQ];
       bad |= !(fabs(piv) > 0.0);
       const double inv = 1.0 / piv;
-      if (c == ko) a[ks][k] = inv;
+      if (wf && c == ko) a[ks][k] = inv;
 #pragma unroll
       for (int s = 0; s < S; s++) {
         if (s < ks) continue;
-        const bool mine = (s > ks) || (c > ko);  // row 4s+c is below the pivot row
+        const bool mine = wf && ((s > ks) || (c > ko));  // row 4s+c is below the pivot row
         if (mine) {
           const double l = a[s][k] * inv;
           lmax = max(lmax, hi_abs(l));
@@ -208,6 +215,11 @@ struct QuadLU {
 
   // dgesl without interchanges: b[s] = my components of the right-hand side / solution
   __device__ __forceinline__ void solve(int c, unsigned gmask, double (&b)[S]) const {
+    fwd_solve(c, gmask, b);
+    back_solve(c, gmask, b);
+  }
+  // forward half (k ascending, axpy form)
+  __device__ __forceinline__ void fwd_solve(int c, unsigned gmask, double (&b)[S]) const {
 #pragma unroll
     for (int k = 0; k < NEQ; k++) {
       const int ko = k & 3, ks = k >> 2;
@@ -218,7 +230,6 @@ struct QuadLU {
         if ((s > ks) || (c > ko)) b[s] = fma_(-a[s][k], bk, b[s]);
       }
     }
-    back_solve(c, gmask, b);
   }
   // backward half only (the forward half was fused into factor())
   __device__ __forceinline__ void back_solve(int c, unsigned gmask, double (&b)[S]) const {

@@ -9,7 +9,9 @@ namespace bz {
 // All warps of a block meet at ONE barrier per loop trip (= per step attempt): that keeps them in
 // the same part of the ~100 KB loop body, so instruction-cache lines fetched by one warp are reused
 // by the others (unsynchronised warps thrashed the instruction cache: profiles/README.md).
-template <class Net, int BLOCK, int MINB>
+// REUSE: the Newton-matrix policy of bz_set_policy(net, 1) (a separate instantiation: the default kernel
+// is compiled without any of it).
+template <class Net, int BLOCK, int MINB, bool REUSE>
 __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, BurnArgs A) {
   constexpr int QUAD_THREADS = BLOCK;
   constexpr int NEQ = Net::NEQ, N = Net::N, K = Net::K, S = Net::S;
@@ -157,7 +159,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
                 m.Z(0, BZQ_I(s)) = y[s];
               }
             __syncwarp(gmask);
-            Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, 0.0, f, lu.a);
+            Net::template eval_quad<true, true>(coef, fac, rho, m.ysh(), m.lam(), c, gmask, 0.0, 0.0, true, f, lu.a);
             BZQ_ADD_SRC(f);
             BZQ_COUNT(CN_INIT);
             // exact second derivative y'' = J f for the first step size
@@ -185,6 +187,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             q = 1, nqwait = 2, nst = 0;
             BZQ_QS = 0, BZQ_NTAU = 0;
             BZQ_T = 0.0, BZQ_ETAMAX = ETAMX1, BZQ_HSAV = 0.0;
+            if (REUSE) m.pint(0) = 0, m.pint(1) = 0, m.sc(Mem::SC_GAMP) = 0.0;
             if (c == 0) {
 #pragma unroll
               for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;
@@ -205,6 +208,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             q = 1, nqwait = 2, nst = 0;
             BZQ_QS = 0, BZQ_NTAU = 0;
             BZQ_T = 0.0, BZQ_ETAMAX = ETAMX1, BZQ_HSAV = 0.0;
+            if (REUSE) m.pint(0) = 0, m.pint(1) = 0, m.sc(Mem::SC_GAMP) = 0.0;
             if (c == 0) {
 #pragma unroll
               for (int i = 0; i <= QMAX; i++) m.sc(Mem::SC_TAU + i) = 0.0;

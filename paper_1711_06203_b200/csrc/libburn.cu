@@ -56,14 +56,16 @@ struct QuadVariant {
   const char *name;
   unsigned long long topo_hash;
   int neq, K, smem_bytes, block;
-  QuadKernelFn fn;
+  QuadKernelFn fn;        // policy 0: fresh Jacobian and LU on every attempt (the default, BZ-BDF v1)
+  QuadKernelFn fn_reuse;  // policy 1: VODE-style reuse of the factorised Newton matrix (BZ-BDF v2)
 };
 template <class Net, int BLOCK, int MINB>
 QuadVariant make_quad(const char *name) {
   const int tab = (4 * Net::K + Net::N + 1) & ~1;
   return {name, Net::TOPO_HASH, Net::NEQ, Net::K,
           (int)sizeof(double) * (tab + bz::QuadMem<Net::NEQ, Net::K>::SIZE * (BLOCK / 4)), BLOCK,
-          (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB>};
+          (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB, false>,
+          (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB, true>};
 }
 // one block of 384 threads per SM (<= 168 registers): all 12 warps share one barrier per trip = one
 // instruction stream (3 blocks of 128 threads were 1.8x slower, profiles/README.md)
@@ -128,7 +130,7 @@ const Variant *pick_variant(int n) {
 namespace {
 constexpr int ST_MAXN = 31, ST_MAXK = 256;
 constexpr size_t ST_HDR = 256;  // 16 x u64 (queue head, 8 counters), padded to the alignment
-constexpr int ST_DBL_CAP = 5 * ST_MAXK + ST_MAXN + 4 * ST_MAXK + 1;                  // doubles (even)
+constexpr int ST_DBL_CAP = 5 * ST_MAXK + ST_MAXN + 4 * ST_MAXK + ST_MAXK + 1;        // doubles (even)
 constexpr int ST_INT_CAP = 4 * ST_MAXK + 2 * (ST_MAXN + 1) + 4 * ST_MAXK + 3 * ST_MAXK;  // ints
 static_assert(ST_HDR + 8 * (size_t)ST_DBL_CAP + 4 * (size_t)ST_INT_CAP <= BZ_STATIC_SCRATCH_BYTES,
               "static scratch too small for the ABI's largest network");
@@ -165,6 +167,7 @@ struct StaticFlat {
   double dbl[ST_DBL_CAP];
   int itab[ST_INT_CAP];
   int ndbl, nint, nterm, ncl;
+  int has_rexp;  // the descriptor carries density exponents: rexp[K] follows sp_dy in dbl
 };
 
 int static_flatten(const bz_net_desc *d, StaticFlat &F) {
@@ -218,6 +221,9 @@ int static_flatten(const bz_net_desc *d, StaticFlat &F) {
     }
   }
   for (int i = 0; i < N; i++) aion[i] = d->aion[i];
+  if (d->rate_rho_exp)
+    for (int k = 0; k < K; k++)
+      if (!std::isfinite(d->rate_rho_exp[k])) return BZ_ERR_NETWORK;
   // CSR by species, entries in ascending k (second pass fills in k order)
   int sp_off[ST_MAXN + 2], cl_off[ST_MAXN + 2], sp_pos[ST_MAXN + 1], cl_pos[ST_MAXN + 1];
   sp_off[0] = cl_off[0] = 0;
@@ -229,7 +235,10 @@ int static_flatten(const bz_net_desc *d, StaticFlat &F) {
   }
   const int nterm = sp_off[N], ncl = cl_off[N];
   F.nterm = nterm; F.ncl = ncl;
-  F.ndbl = 5 * K + N + nterm;
+  F.has_rexp = d->rate_rho_exp ? 1 : 0;
+  F.ndbl = 5 * K + N + nterm + (F.has_rexp ? K : 0);
+  if (F.has_rexp)
+    for (int k = 0; k < K; k++) F.dbl[5 * K + N + nterm + k] = d->rate_rho_exp[k];
   F.nint = 4 * K + (N + 1) + nterm + (N + 1) + ncl;
   if (F.ndbl > ST_DBL_CAP || F.nint > ST_INT_CAP) return BZ_ERR_SIZE;
   int *t_rp = F.itab, *t_spoff = t_rp + 4 * K, *t_spk = t_spoff + (N + 1);
@@ -267,6 +276,8 @@ struct bz_net {
   int device;      // the device that was current at net_create: a handle belongs to ONE device
   int static_sched;  // bz_set_schedule: 0 = work queue (a2), 1 = static round-robin assignment
   int mxstep, mxnef, mxncf;  // bz_set_limits
+  int policy;                // bz_set_policy: 0 fresh matrix every attempt, 1 reuse
+  int quad_grid_reuse;
   // staging for burn_zones_host
   double *st_in, *st_out;
   int32_t *st_nsteps;
@@ -315,6 +326,7 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   h->dev.fac = 9.648533212331e17 / d->cv;
   h->dev.dbl = h->d_dbl; h->dev.itab = h->d_int;
   h->dev.ndbl = F.ndbl; h->dev.nint = F.nint;
+  h->dev.has_rexp = F.has_rexp;
   h->fac = h->dev.fac;
 
   // ---- launch geometry: persistent grid, blocks/SM from the occupancy calculator -----------------
@@ -342,6 +354,7 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   const unsigned long long th = topology_hash(d);
   for (const QuadVariant &v : kQuad)
     if (v.topo_hash == th && v.neq == n && v.K == K) h->quad = &v;
+  if (F.has_rexp) h->quad = nullptr;  // the generated code has no density exponents: generic kernel
   if (h->quad) {
     // coefficient table of the generated code: lnA[K] n[K] B[K] Q[K] aion[N]
     double qc[4 * ST_MAXK + ST_MAXN];
@@ -361,8 +374,16 @@ int net_create(const bz_net_desc *d, bz_net **out) {
       return fail(BZ_ERR_CUDA);
     if (qb < 1) return fail(BZ_ERR_NOMEM);
     h->quad_grid = sms * qb;
+    if (!cuda_ok(cudaFuncSetAttribute((const void *)h->quad->fn_reuse, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
+      return fail(BZ_ERR_CUDA);
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&qb, (const void *)h->quad->fn_reuse, h->quad->block,
+                                                               h->quad->smem_bytes)))
+      return fail(BZ_ERR_CUDA);
+    if (qb < 1) return fail(BZ_ERR_NOMEM);
+    h->quad_grid_reuse = sms * qb;
     const size_t per_quad = (size_t)n * n + 2 * n;
-    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * h->quad_grid * (h->quad->block / 4) * sizeof(double))))
+    const int gmax = h->quad_grid > h->quad_grid_reuse ? h->quad_grid : h->quad_grid_reuse;
+    if (!cuda_ok(cudaMalloc(&h->d_quad_scratch, per_quad * gmax * (h->quad->block / 4) * sizeof(double))))
       return fail(BZ_ERR_CUDA);
   }
   *out = h;
@@ -396,6 +417,12 @@ int bz_set_schedule(bz_net *h, int kind) {
   if (!h) return BZ_ERR_NULL;
   if (kind != 0 && kind != 1) return BZ_ERR_SIZE;
   h->static_sched = kind;
+  return BZ_OK;
+}
+int bz_set_policy(bz_net *h, int kind) {
+  if (!h) return BZ_ERR_NULL;
+  if (kind != 0 && kind != 1) return BZ_ERR_SIZE;
+  h->policy = kind;
   return BZ_OK;
 }
 int bz_set_limits(bz_net *h, int32_t mxstep, int32_t mxnef, int32_t mxncf) {
@@ -434,6 +461,7 @@ int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double 
   if (nz == 0) return BZ_OK;
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
   if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
+  if (h->policy == 1 && !use_quad(h)) return BZ_ERR_UNSUPPORTED;  // reuse exists in the specialised kernels only
   const int drc = check_device(h);
   if (drc != BZ_OK) return drc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -452,9 +480,11 @@ int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double 
     qn.gscratch = h->d_quad_scratch;
     const int zpb = h->quad->block / 4;
     const long long blocks_needed = (nz + zpb - 1) / zpb;
-    const int grid = (int)(blocks_needed < h->quad_grid ? blocks_needed : h->quad_grid);
+    const int full = h->policy == 1 ? h->quad_grid_reuse : h->quad_grid;
+    const int grid = (int)(blocks_needed < full ? blocks_needed : full);
+    const QuadKernelFn fn = h->policy == 1 ? h->quad->fn_reuse : h->quad->fn;
     void *qargs[] = {(void *)&qn, (void *)&a};
-    BZ_CUDA(cudaLaunchKernel((const void *)h->quad->fn, dim3(grid), dim3(h->quad->block), qargs,
+    BZ_CUDA(cudaLaunchKernel((const void *)fn, dim3(grid), dim3(h->quad->block), qargs,
                              (size_t)h->quad->smem_bytes, st));
     return BZ_OK;
   }
@@ -571,6 +601,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   dn.fac = 9.648533212331e17 / d->cv;
   dn.dbl = d_dbl; dn.itab = d_int;
   dn.ndbl = F.ndbl; dn.nint = F.nint;
+  dn.has_rexp = F.has_rexp;
   bz::BurnArgs a;
   a.src_T = nullptr; a.src_X = nullptr;
   a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;

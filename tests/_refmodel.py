@@ -27,13 +27,17 @@ class RefModel:
         n = self.net
         return n.rate_A * T9 ** n.rate_n * np.exp(-n.rate_B / np.cbrt(T9))
 
+    def rho_factor(self, rho):
+        e = getattr(self.net, "rate_rho_exp", None)
+        return 1.0 if e is None else rho ** np.asarray(e)
+
     def rate(self, k, rho, Y, lam):
         r = self.reac[k]
         mag = lam[k] * rho ** (len(r) - 1) * self.sym[k] * np.prod([abs(Y[a]) for a in r])
         return -mag if any(Y[a] < 0 for a in r) else mag      # reading s19 (odd extension)
 
     def f(self, rho, y):
-        lam = self.lam(y[self.N])
+        lam = self.lam(y[self.N]) * self.rho_factor(rho)
         out = np.zeros(self.N + 1)
         for k in range(self.K):
             R = self.rate(k, rho, y, lam)

@@ -15,5 +15,7 @@ from .configs import (  # noqa: F401
     first_order_decay_network,
     aprox13_like_network,
     make_aprox13_like_workload,
+    urca9_like_network,
+    make_urca9_like_workload,
     sha256_of,
 )

@@ -49,6 +49,7 @@ class Network:
     rate_B: np.ndarray
     q_mev: np.ndarray
     cv: float = CV
+    rate_rho_exp: Optional[np.ndarray] = None    # [K] density exponents of weak rates (None = none)
 
     @property
     def nspec(self) -> int:
@@ -235,6 +236,69 @@ def make_aprox13_like_workload(nz: int, seed: int = 6, dt: float = 1e-6) -> Work
     X = np.zeros((13, nz))
     X[[0, 1, 2, 5, 12]] = g / g.sum(axis=0)
     return Workload(6, net, 10.0 ** (6.0 + 2.0 * u_rho), 1e9 + 3e9 * u_T, X, dt, nz_full=nz)
+
+
+def urca9_like_network(seed: int = 9) -> Network:
+    """A 9-species network in the style of the Urca network the paper's Fig. 5 ran ("the 9-isotope Urca
+    network is used for our Urca simulations"): free neutrons and
+    protons, the carbon-burning channels that emit alpha / p / n, and an A = 23 Urca pair linked by
+    WEAK, first-order reactions whose rates depend on density and temperature (electron capture grows
+    with rho, beta decay is blocked by it).  The real network takes those rates from tables in
+    (rho Y_e, T), which are not available and are not reproduced: here lambda = A T9^n exp(-B/T9^(1/3))
+    rho^e with synthetic coefficients from ``default_rng(seed)`` -- capture-like links e in [1, 2] and
+    A = 10^(-21+3u)... chosen so that lambda ~ 1e5..1e7 /s around rho = 1e9; decay-like links e in
+    [-1, -0.3].  12 reactions, four-entry stoichiometry, reactions with negative Q.  Runs on the generic
+    cooperative kernel."""
+    rng = np.random.default_rng(seed)
+    sp = ["n", "p", "He4", "C12", "O16", "Ne20", "Ne23", "Na23", "Mg23"]
+    aion = np.array([1.0, 1.0, 4.0, 12.0, 16.0, 20.0, 23.0, 23.0, 23.0])
+    n_, p_, he, c12, o16, ne20, ne23, na23, mg23 = range(9)
+    strong = [
+        ([c12, c12], [(c12, -2.0), (ne20, +1.0), (he, +1.0)]),               # C12 + C12 -> Ne20 + a
+        ([c12, c12], [(c12, -2.0), (na23, +1.0), (p_, +1.0)]),               # C12 + C12 -> Na23 + p
+        ([c12, c12], [(c12, -2.0), (mg23, +1.0), (n_, +1.0)]),               # C12 + C12 -> Mg23 + n
+        ([c12, he], [(c12, -1.0), (he, -1.0), (o16, +1.0)]),                 # C12 (a,g) O16
+        ([o16, he], [(o16, -1.0), (he, -1.0), (ne20, +1.0)]),                # O16 (a,g) Ne20
+        ([na23, p_], [(na23, -1.0), (p_, -1.0), (ne20, +1.0), (he, +1.0)]),  # Na23 (p,a) Ne20
+        ([mg23, n_], [(mg23, -1.0), (n_, -1.0), (na23, +1.0), (p_, +1.0)]),  # Mg23 (n,p) Na23
+    ]
+    weak = [   # (reactant, product, capture-like?)
+        (ne23, na23, False),   # beta decay of the Urca pair
+        (na23, ne23, True),    # electron capture of the Urca pair
+        (mg23, na23, True),
+        (n_, p_, False),
+        (p_, n_, True),
+    ]
+    reactants = [r for r, _ in strong] + [[a] for a, _, _ in weak]
+    stoich = [s for _, s in strong] + [[(a, -1.0), (b, +1.0)] for a, b, _ in weak]
+    K = len(reactants)
+    A, n, B, Q = _coeffs(rng, len(strong))
+    u = rng.random((4, len(weak)))
+    cap = np.array([c for _, _, c in weak])
+    e_w = np.where(cap, 1.0 + u[0], -1.0 + 0.7 * u[0])
+    # lambda ~ 10^(5..7) /s at rho = 1e9, T9 = 1:  A = 10^(5 + 2u - 9 e)
+    A_w = 10.0 ** (5.0 + 2.0 * u[1] - 9.0 * e_w)
+    n_w = -1.0 + 2.0 * u[2]
+    B_w = 5.0 * u[3]
+    Q_w = np.where(cap, -1.0, +1.0) * (0.5 + 4.0 * rng.random(len(weak)))
+    reactant, sid, sdy = _pack(K, reactants, stoich)
+    return Network("urca9like", sp, aion, reactant, sid, sdy, np.concatenate([A, A_w]), np.concatenate([n, n_w]),
+                   np.concatenate([B, B_w]), np.concatenate([Q, Q_w]),
+                   rate_rho_exp=np.concatenate([np.zeros(len(strong)), e_w]))
+
+
+def make_urca9_like_workload(nz: int, seed: int = 9, dt: float = 1e-6) -> Workload:
+    """``nz`` zones for ``urca9_like_network``: rho log-uniform [1e8, 1e10] (around an Urca threshold),
+    T uniform [5e8, 3e9], X = Dirichlet(1) over C12, O16, Ne23, Na23 with 1e-3 of free n and p each."""
+    net = urca9_like_network(seed)
+    rng = np.random.default_rng(seed + 1000)
+    u_rho, u_T = rng.random(nz), rng.random(nz)
+    g = -np.log1p(-rng.random((4, nz)))
+    X = np.zeros((9, nz))
+    X[[3, 4, 6, 7]] = 0.998 * g / g.sum(axis=0)
+    X[0] = 1e-3
+    X[1] = 1e-3
+    return Workload(7, net, 10.0 ** (8.0 + 2.0 * u_rho), 5e8 + 2.5e9 * u_T, X, dt, nz_full=nz)
 
 
 def first_order_decay_network(lam: float, q_mev: float = 0.0) -> Network:
