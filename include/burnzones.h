@@ -68,6 +68,15 @@ typedef struct {
                                 "the 9-isotope Urca network").  Evaluated
                                 inside the exponent: arg_k += e_k * ln(rho).  Finite values; NULL = none.
                                 Networks that carry it run on the generic cooperative kernel.            */
+  const double *zion;        /* [N] or NULL: charges Z_i.  Non-NULL selects an analytic equation of state for
+                                the specific heat, evaluated with every right-hand side (
+                                "supports arbitrary equations of state"), and
+                                `cv` is ignored:
+                                  c_v(rho,T,Y) = 1.5 R (eos_extra + sum_i (1+Z_i) Y_i) + 4 a T^3 / rho
+                                (ideal ions and electrons + radiation; R = 8.31446261815324e7 erg/mol/K,
+                                a = 7.565733250e-15 erg/cm^3/K^4).  Z_i >= 0, finite.  Generic kernel only. */
+  double eos_extra;          /* mol/g, >= 0: sum (1+Z_i) Y_i over species that are NOT evolved (read only
+                                when zion != NULL)                                                        */
 } bz_net_desc;
 
 /* Validate, flatten and upload a network.  *out receives the handle.  A handle belongs to the

@@ -18,6 +18,8 @@
 
 /* ---- constants of C.1 / C.2 ------------------------------------------------------- */
 #define NA_MEV 9.648533212331e17 /* N_A * 1 MeV in erg/mol */
+#define RGAS 8.31446261815324e7  /* N_A k_B, erg/mol/K (analytic EOS) */
+#define ARAD 7.565733250e-15     /* radiation constant a, erg/cm^3/K^4 */
 #define QMAX 5
 #define MAXCOR 3
 #define NTOL 0.1
@@ -99,6 +101,9 @@ typedef struct {
   double lnA[ORC_KMAX], en[ORC_KMAX], B[ORC_KMAX], Q[ORC_KMAX], invsym[ORC_KMAX];
   int has_rexp;            /* the descriptor carries density exponents */
   double rexp[ORC_KMAX];
+  int eos;                 /* 1: c_v from the analytic EOS, evaluated with every right-hand side */
+  double zp1[ORC_NMAX];    /* 1 + Z_i */
+  double eos_extra;
   double fac;              /* N_A MeV / c_v                          */
 } Net;
 
@@ -107,8 +112,15 @@ static int net_init(Net *nt, const orc_net_desc *d) {
   nt->N = d->nspec;
   nt->n = d->nspec + 1;
   nt->K = d->nreac;
-  if (!(d->cv > 0.0)) return -3;
-  nt->fac = NA_MEV / d->cv;
+  nt->eos = (d->zion != NULL);
+  if (!nt->eos && !(d->cv > 0.0)) return -3;
+  nt->fac = nt->eos ? 0.0 : NA_MEV / d->cv;
+  nt->eos_extra = nt->eos ? d->eos_extra : 0.0;
+  if (nt->eos && (!isfinite(d->eos_extra) || d->eos_extra < 0.0)) return -3;
+  for (int i = 0; i < d->nspec && nt->eos; i++) {
+    if (!isfinite(d->zion[i]) || d->zion[i] < 0.0) return -3;
+    nt->zp1[i] = 1.0 + d->zion[i];
+  }
   nt->has_rexp = (d->rate_rho_exp != NULL);
   for (int i = 0; i < nt->N; i++) {
     if (!(d->aion[i] > 0.0)) return -3;
@@ -240,9 +252,27 @@ static void rates(const Net *nt, double rho, const double *y, double *f, double 
     }
     JT[TI] = fma(nt->Q[k], dRdT, JT[TI]);
   }
-  f[TI] = nt->fac * sT;
-  if (J)
-    for (int j = 0; j < n; j++) J[TI * n + j] = nt->fac * JT[j];
+  if (!nt->eos) {
+    f[TI] = nt->fac * sT;
+    if (J)
+      for (int j = 0; j < n; j++) J[TI * n + j] = nt->fac * JT[j];
+    return;
+  }
+  /* analytic EOS: c_v = 1.5 R (extra + sum_i (1+Z_i) Y_i) + 4 a T^3 / rho, raw Y, i ascending;
+   * dT/dt = (N_A MeV / c_v) sum_k Q_k R_k; the temperature row of J gains -f_T (dc_v/dy_j) / c_v */
+  double ysum = nt->eos_extra;
+  for (int i = 0; i < N; i++) ysum = fma(nt->zp1[i], y[SP(i)], ysum);
+  const double T2 = T * T;
+  const double invrho = 1.0 / rho;
+  const double cv = fma(1.5 * RGAS, ysum, ((4.0 * ARAD) * (T2 * T)) * invrho);
+  const double invcv = 1.0 / cv;
+  const double facv = NA_MEV * invcv;
+  f[TI] = facv * sT;
+  if (J) {
+    const double g = f[TI] * invcv;
+    J[TI * n + TI] = fma(-g, ((12.0 * ARAD) * T2) * invrho, facv * JT[TI]);
+    for (int i = 0; i < N; i++) J[TI * n + SP(i)] = fma(-g, (1.5 * RGAS) * nt->zp1[i], facv * JT[SP(i)]);
+  }
 }
 
 /* ---- dense LU, LINPACK dgefa/dgesl order (step a5/a6; C.5 item 4) ------------------- */

@@ -53,6 +53,13 @@ typedef struct {
    * network"): lambda_k is multiplied by rho^rate_rho_exp[k] ON TOP of the rho^(m-1) of
    * the rate law, evaluated inside the exponent: arg_k += rate_rho_exp[k] * ln(rho).  NULL = none. */
   const double *rate_rho_exp; /* [K] or NULL */
+  /* optional analytic equation of state for the specific heat ("supports arbitrary
+   * equations of state").  zion != NULL selects it and `cv` is ignored:
+   *   c_v(rho, T, Y) = 1.5 R (eos_extra + sum_i (1 + Z_i) Y_i) + 4 a T^3 / rho     [erg/g/K]
+   * (ideal ions and electrons, radiation; R = 8.31446261815324e7 erg/mol/K, a = 7.565733250e-15
+   * erg/cm^3/K^4).  eos_extra [mol/g]: the same sum over species that are not evolved (config 1's O16). */
+  const double *zion;         /* [N] charges Z_i, or NULL */
+  double eos_extra;
 } orc_net_desc;
 
 typedef struct {

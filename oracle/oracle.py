@@ -16,7 +16,8 @@ _ip = C.POINTER(C.c_int32)
 class _Desc(C.Structure):
     _fields_ = [("nspec", C.c_int32), ("nreac", C.c_int32), ("aion", _dp), ("reactant", _ip),
                 ("stoich_id", _ip), ("stoich_dy", _dp), ("rate_A", _dp), ("rate_n", _dp),
-                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double), ("rate_rho_exp", _dp)]
+                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double), ("rate_rho_exp", _dp),
+                ("zion", _dp), ("eos_extra", C.c_double)]
 
 
 class _Opts(C.Structure):
@@ -88,6 +89,10 @@ def _desc(net):
         rate_B=np.ascontiguousarray(net.rate_B, dtype=np.float64),
         q_mev=np.ascontiguousarray(net.q_mev, dtype=np.float64),
     )
+    zion = getattr(net, "zion", None)
+    if zion is not None:
+        keep["zion"] = np.ascontiguousarray(zion, dtype=np.float64)
+        assert keep["zion"].shape == keep["aion"].shape
     rexp = getattr(net, "rate_rho_exp", None)
     if rexp is not None:
         keep["rate_rho_exp"] = np.ascontiguousarray(rexp, dtype=np.float64)
@@ -95,7 +100,8 @@ def _desc(net):
     d = _Desc(int(keep["aion"].shape[0]), int(keep["rate_A"].shape[0]), _d(keep["aion"]),
               _i(keep["reactant"]), _i(keep["stoich_id"]), _d(keep["stoich_dy"]), _d(keep["rate_A"]),
               _d(keep["rate_n"]), _d(keep["rate_B"]), _d(keep["q_mev"]), float(net.cv),
-              _d(keep["rate_rho_exp"]) if rexp is not None else None)
+              _d(keep["rate_rho_exp"]) if rexp is not None else None,
+              _d(keep["zion"]) if zion is not None else None, float(getattr(net, "eos_extra", 0.0) or 0.0))
     return d, keep
 
 

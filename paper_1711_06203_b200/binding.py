@@ -31,7 +31,8 @@ class BurnError(RuntimeError):
 class _Desc(C.Structure):
     _fields_ = [("nspec", C.c_int32), ("nreac", C.c_int32), ("aion", _dp), ("reactant", _ip),
                 ("stoich_id", _ip), ("stoich_dy", _dp), ("rate_A", _dp), ("rate_n", _dp),
-                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double), ("rate_rho_exp", _dp)]
+                ("rate_B", _dp), ("q_mev", _dp), ("cv", C.c_double), ("rate_rho_exp", _dp),
+                ("zion", _dp), ("eos_extra", C.c_double)]
 
 
 def library_path() -> str:
@@ -147,7 +148,7 @@ def _i32(a):
 
 
 def net_create(net=None, *, aion=None, reactant=None, stoich_id=None, stoich_dy=None, rate_A=None,
-               rate_n=None, rate_B=None, q_mev=None, cv=None, rate_rho_exp=None) -> Net:
+               rate_n=None, rate_B=None, q_mev=None, cv=None, rate_rho_exp=None, zion=None, eos_extra=None) -> Net:
     """net_create(rates, Q-values, isotope masses): `net` is any object with those fields
     (e.g. workloads.Network), or pass them as keywords."""
     g = (lambda k, v: v if v is not None else getattr(net, k))
@@ -166,7 +167,9 @@ def net_create(net=None, *, aion=None, reactant=None, stoich_id=None, stoich_dy=
               keep["stoich_id"].ctypes.data_as(_ip), keep["stoich_dy"].ctypes.data_as(_dp),
               keep["rate_A"].ctypes.data_as(_dp), keep["rate_n"].ctypes.data_as(_dp),
               keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp),
-              float(g("cv", cv)), _rexp_ptr(rexp, K, keep))
+              float(g("cv", cv)), _rexp_ptr(rexp, K, keep),
+              _zion_ptr(zion if zion is not None else getattr(net, "zion", None), N, keep),
+              float(eos_extra if eos_extra is not None else (getattr(net, "eos_extra", 0.0) or 0.0)))
     h = C.c_void_p()
     _check(_L().net_create(C.byref(d), C.byref(h)), "net_create")
     return Net(h, N, K)
@@ -180,6 +183,16 @@ def _rexp_ptr(rexp, K, keep):
     if keep["rate_rho_exp"].shape != (K,):
         raise ValueError("rate_rho_exp must be [K]")
     return keep["rate_rho_exp"].ctypes.data_as(_dp)
+
+
+def _zion_ptr(zion, N, keep):
+    """Optional charges [N] (select the analytic EOS for c_v) -> pointer, NULL when absent."""
+    if zion is None:
+        return None
+    keep["zion"] = _f64(zion)
+    if keep["zion"].shape != (N,):
+        raise ValueError("zion must be [N]")
+    return keep["zion"].ctypes.data_as(_dp)
 
 
 def net_destroy(net: Net) -> None:
@@ -309,7 +322,8 @@ def burn_zones_static(desc, rho, T, X, dt, rtol, atol, T_out, X_out, nsteps, str
               keep["stoich_id"].ctypes.data_as(_ip), keep["stoich_dy"].ctypes.data_as(_dp),
               keep["rate_A"].ctypes.data_as(_dp), keep["rate_n"].ctypes.data_as(_dp),
               keep["rate_B"].ctypes.data_as(_dp), keep["q_mev"].ctypes.data_as(_dp), float(desc.cv),
-              _rexp_ptr(getattr(desc, "rate_rho_exp", None), K, keep))
+              _rexp_ptr(getattr(desc, "rate_rho_exp", None), K, keep),
+              _zion_ptr(getattr(desc, "zion", None), N, keep), float(getattr(desc, "eos_extra", 0.0) or 0.0))
     p = lambda t: C.c_void_p(t.data_ptr())
     _check(_L().burn_zones_static(C.byref(d), nz, p(rho), p(T), p(X), float(dt), float(rtol), float(atol),
                                   p(T_out), p(X_out), p(nsteps), _stream_ptr(stream)), "burn_zones_static")

@@ -28,6 +28,8 @@ constexpr double BIAS1 = 4.0, BIAS2 = 6.0, BIAS3 = 10.0, ADDON = 1e-6, THRESH = 
 constexpr double ETAMIN = 0.1, ETAMXF = 0.2, ETAMX1 = 1e4, ETAMAX = 2.0, SLIVER = 1e-6;
 // Newton-matrix reuse (bz_set_policy 1, "BZ-BDF v2"): refactor when |gamma/gamma_P - 1|
 // exceeds CCMAX or MSBP steps were accepted since the last factorisation
+// analytic EOS for c_v: N_A k_B [erg/mol/K], radiation constant a [erg/cm^3/K^4], N_A MeV
+constexpr double RGAS = 8.31446261815324e7, ARAD = 7.565733250e-15, NA_MEV = 9.648533212331e17;
 constexpr double CCMAX = 0.3;
 constexpr int MSBP = 20;
 
@@ -39,6 +41,8 @@ struct DevNet {
   const int *itab;        // rp[4K] sp_off[N+1] sp_k[nterm] cl_off[N+1] cl_ks[ncl]
   int ndbl, nint;
   int has_rexp;           // density exponents of weak rates present (bz_net_desc.rate_rho_exp)
+  int eos;                // c_v from the analytic EOS (bz_net_desc.zion): zp1[N] follows rexp in dbl; fac unused
+  double eos_extra;
 };
 
 struct BurnArgs {

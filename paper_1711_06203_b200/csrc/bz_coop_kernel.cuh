@@ -15,6 +15,8 @@ struct Group {
   double fac, inv_n;
   const double *lnA, *en, *B, *Q, *invsym, *aion, *sp_dy;
   const double *rexp;  // density exponents of weak rates, or nullptr
+  const double *zp1;   // 1 + Z_i: c_v from the analytic EOS, or nullptr (constant c_v in fac)
+  double eos_extra;
   const int *rp, *sp_off, *sp_k, *cl_off, *cl_ks;
   // per-group scratch in shared memory
   double *ysh, *R, *dRdT, *dRdY, *M, *urow, *xs;
@@ -152,6 +154,18 @@ struct Group {
       }
     }
     sync();
+    // analytic EOS: c_v = 1.5 R (extra + sum_i (1+Z_i) Y_i) + 4 a T^3 / rho, raw Y, i ascending; every lane
+    // computes it (uniform code, identical bits); facv replaces the constant fac
+    double facv = fac, invcv = 0.0, T2 = 0.0, invrho = 0.0;
+    if (zp1) {
+      double ysum = eos_extra;
+      for (int i = 0; i < N; i++) ysum = fma_(zp1[i], ysh[i + 1], ysum);
+      T2 = T * T;
+      invrho = 1.0 / rho;
+      const double cv = fma_(1.5 * RGAS, ysum, ((4.0 * ARAD) * (T2 * T)) * invrho);
+      invcv = 1.0 / cv;
+      facv = NA_MEV * invcv;
+    }
     double f = 0.0, jt0 = 0.0;
     const int sp = lig - 1;  // my species (lanes 1..N); lane 0 owns T
     if (lig >= 1 && lig <= N) {
@@ -169,7 +183,7 @@ struct Group {
       } else {
         for (int k = 0; k < K; k++) s = fma_(Q[k], R[k], s);
       }
-      f = fac * s;
+      f = facv * s;
     }
     if (WITH_J) {
       double *row = M + lig * LD;
@@ -199,7 +213,14 @@ struct Group {
         jt = jt0;  // summed alongside f above (same k-ascending fma chain)
       }
       sync();  // rows of the species are complete before the T row is written
-      if (lig < n) M[lig] = fac * jt;  // row 0 = temperature equation
+      if (zp1) {
+        // dT/dt = facv s: the row gains -f_T (dc_v/dy_j) / c_v, dc_v/dT = 12 a T^2/rho, dc_v/dY_j = 1.5 R (1+Z_j)
+        const double gq = bcast(f, 0) * invcv;
+        const double dcv = (lig == 0) ? ((12.0 * ARAD) * T2) * invrho : ((lig <= N) ? (1.5 * RGAS) * zp1[sp] : 0.0);
+        if (lig < n) M[lig] = fma_(-gq, dcv, facv * jt);
+      } else if (lig < n) {
+        M[lig] = fac * jt;  // row 0 = temperature equation
+      }
       sync();
     }
     if (has_src) f = f + src;

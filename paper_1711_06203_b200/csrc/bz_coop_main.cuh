@@ -35,6 +35,8 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
   g.lnA = s_dbl; g.en = s_dbl + K; g.B = s_dbl + 2 * K; g.Q = s_dbl + 3 * K; g.invsym = s_dbl + 4 * K;
   g.aion = s_dbl + 5 * K; g.sp_dy = s_dbl + 5 * K + N;
   g.rexp = net.has_rexp ? s_dbl + 5 * K + N + net.nterm : nullptr;
+  g.zp1 = net.eos ? s_dbl + 5 * K + N + net.nterm + (net.has_rexp ? K : 0) : nullptr;
+  g.eos_extra = net.eos_extra;
   g.rp = s_int; g.sp_off = s_int + 4 * K; g.sp_k = g.sp_off + (N + 1);
   g.cl_off = g.sp_k + net.nterm; g.cl_ks = g.cl_off + (N + 1);
   {

@@ -130,7 +130,7 @@ const Variant *pick_variant(int n) {
 namespace {
 constexpr int ST_MAXN = 31, ST_MAXK = 256;
 constexpr size_t ST_HDR = 256;  // 16 x u64 (queue head, 8 counters), padded to the alignment
-constexpr int ST_DBL_CAP = 5 * ST_MAXK + ST_MAXN + 4 * ST_MAXK + ST_MAXK + 1;        // doubles (even)
+constexpr int ST_DBL_CAP = 5 * ST_MAXK + ST_MAXN + 4 * ST_MAXK + ST_MAXK + ST_MAXN;  // doubles (even)
 constexpr int ST_INT_CAP = 4 * ST_MAXK + 2 * (ST_MAXN + 1) + 4 * ST_MAXK + 3 * ST_MAXK;  // ints
 static_assert(ST_HDR + 8 * (size_t)ST_DBL_CAP + 4 * (size_t)ST_INT_CAP <= BZ_STATIC_SCRATCH_BYTES,
               "static scratch too small for the ABI's largest network");
@@ -168,11 +168,18 @@ struct StaticFlat {
   int itab[ST_INT_CAP];
   int ndbl, nint, nterm, ncl;
   int has_rexp;  // the descriptor carries density exponents: rexp[K] follows sp_dy in dbl
+  int eos;       // analytic EOS for c_v: zp1[N] = 1 + Z_i follows (after rexp)
 };
 
 int static_flatten(const bz_net_desc *d, StaticFlat &F) {
   const int N = d->nspec, K = d->nreac;
-  if (!(d->cv > 0.0) || !std::isfinite(d->cv)) return BZ_ERR_NETWORK;
+  F.eos = d->zion ? 1 : 0;
+  if (!F.eos && (!(d->cv > 0.0) || !std::isfinite(d->cv))) return BZ_ERR_NETWORK;
+  if (F.eos) {
+    if (!std::isfinite(d->eos_extra) || d->eos_extra < 0.0) return BZ_ERR_NETWORK;
+    for (int i = 0; i < N; i++)
+      if (!std::isfinite(d->zion[i]) || d->zion[i] < 0.0) return BZ_ERR_NETWORK;
+  }
   for (int i = 0; i < N; i++)
     if (!(d->aion[i] > 0.0) || !std::isfinite(d->aion[i])) return BZ_ERR_NETWORK;
   int rp[4 * ST_MAXK] = {0};
@@ -239,6 +246,10 @@ int static_flatten(const bz_net_desc *d, StaticFlat &F) {
   F.ndbl = 5 * K + N + nterm + (F.has_rexp ? K : 0);
   if (F.has_rexp)
     for (int k = 0; k < K; k++) F.dbl[5 * K + N + nterm + k] = d->rate_rho_exp[k];
+  if (F.eos) {
+    for (int i = 0; i < N; i++) F.dbl[F.ndbl + i] = 1.0 + d->zion[i];
+    F.ndbl += N;
+  }
   F.nint = 4 * K + (N + 1) + nterm + (N + 1) + ncl;
   if (F.ndbl > ST_DBL_CAP || F.nint > ST_INT_CAP) return BZ_ERR_SIZE;
   int *t_rp = F.itab, *t_spoff = t_rp + 4 * K, *t_spk = t_spoff + (N + 1);
@@ -323,7 +334,8 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     return fail(BZ_ERR_CUDA);
   if (!cuda_ok(cudaMemset(h->d_scratch, 0, 16 * sizeof(unsigned long long)))) return fail(BZ_ERR_CUDA);
   h->dev.N = N; h->dev.n = n; h->dev.K = K; h->dev.nterm = F.nterm; h->dev.ncl = F.ncl;
-  h->dev.fac = 9.648533212331e17 / d->cv;
+  h->dev.fac = F.eos ? 0.0 : 9.648533212331e17 / d->cv;
+  h->dev.eos = F.eos; h->dev.eos_extra = F.eos ? d->eos_extra : 0.0;
   h->dev.dbl = h->d_dbl; h->dev.itab = h->d_int;
   h->dev.ndbl = F.ndbl; h->dev.nint = F.nint;
   h->dev.has_rexp = F.has_rexp;
@@ -354,7 +366,7 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   const unsigned long long th = topology_hash(d);
   for (const QuadVariant &v : kQuad)
     if (v.topo_hash == th && v.neq == n && v.K == K) h->quad = &v;
-  if (F.has_rexp) h->quad = nullptr;  // the generated code has no density exponents: generic kernel
+  if (F.has_rexp || F.eos) h->quad = nullptr;  // the generated code has neither density exponents nor the EOS
   if (h->quad) {
     // coefficient table of the generated code: lnA[K] n[K] B[K] Q[K] aion[N]
     double qc[4 * ST_MAXK + ST_MAXN];
@@ -598,7 +610,8 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
 
   bz::DevNet dn;
   dn.N = N; dn.n = n; dn.K = K; dn.nterm = F.nterm; dn.ncl = F.ncl;
-  dn.fac = 9.648533212331e17 / d->cv;
+  dn.fac = F.eos ? 0.0 : 9.648533212331e17 / d->cv;
+  dn.eos = F.eos; dn.eos_extra = F.eos ? d->eos_extra : 0.0;
   dn.dbl = d_dbl; dn.itab = d_int;
   dn.ndbl = F.ndbl; dn.nint = F.nint;
   dn.has_rexp = F.has_rexp;

@@ -4,6 +4,8 @@ scipy cross-check).  libm exp/pow, no ordering contract -- agreement is to round
 import numpy as np
 
 NA_MEV = 9.648533212331e17
+RGAS = 8.31446261815324e7
+ARAD = 7.565733250e-15
 
 
 class RefModel:
@@ -43,8 +45,17 @@ class RefModel:
             R = self.rate(k, rho, y, lam)
             for i, d in self.sto[k]:
                 out[i] += d * R
-            out[self.N] += self.fac * self.net.q_mev[k] * R
+            out[self.N] += self.net.q_mev[k] * R
+        out[self.N] *= NA_MEV / self.cv(rho, y)
         return out
+
+    def cv(self, rho, y):
+        """Constant c_v, or the analytic EOS when the network carries charges."""
+        z = getattr(self.net, "zion", None)
+        if z is None:
+            return self.net.cv
+        ysum = getattr(self.net, "eos_extra", 0.0) + np.dot(1.0 + np.asarray(z), y[: self.N])
+        return 1.5 * RGAS * ysum + 4.0 * ARAD * y[self.N] ** 3 / rho
 
     def jac_fd(self, rho, y, rel=1e-6):
         n = self.N + 1

@@ -50,6 +50,8 @@ class Network:
     q_mev: np.ndarray
     cv: float = CV
     rate_rho_exp: Optional[np.ndarray] = None    # [K] density exponents of weak rates (None = none)
+    zion: Optional[np.ndarray] = None            # [N] charges Z_i: selects the analytic EOS for c_v (None = constant cv)
+    eos_extra: float = 0.0                       # mol/g: sum (1 + Z_i) Y_i over species that are not evolved
 
     @property
     def nspec(self) -> int:
