@@ -46,7 +46,8 @@ struct DevNet {
 };
 
 struct BurnArgs {
-  long long nz;
+  long long nz;   // zones of this launch
+  long long ld;   // row stride of X, X_out, src_X in doubles (= nz, except for the chunks of burn_zones_host)
   const double *rho, *T, *X;
   double dt, rtol, atol;
   double *T_out, *X_out;

@@ -16,7 +16,8 @@ struct LuRow {
 
   // a5: in-place LU with partial pivoting, LINPACK tie-break (first maximal |a_ik| in the
   // current row order), rows never move.  Returns false if a pivot column is all zero.
-  __device__ __forceinline__ bool factor(const Group<NEQ, LANES> &g) {
+  template <class G>
+  __device__ __forceinline__ bool factor(const G &g) {
     const int lig = g.lig;
     pos = lig;
     myinv = 0.0;
@@ -61,7 +62,8 @@ struct LuRow {
   }
 
   // a6: solve P x = b (dgesl order).  b = my component on entry, x_lig on return.
-  __device__ __forceinline__ double solve(const Group<NEQ, LANES> &g, double b) const {
+  template <class G>
+  __device__ __forceinline__ double solve(const G &g, double b) const {
 #pragma unroll
     for (int k = 0; k < NEQ; k++) {
       const double bk = g.bcast(b, pivot_lane(k));

@@ -4,7 +4,10 @@
 
 namespace bz {
 
-template <int NEQ, int LANES>
+// EXT: the optional model extensions -- density exponents of weak rates and c_v from the
+// analytic EOS -- are compiled into a separate instantiation, so that networks without
+// them run the kernel without a trace of either (they cost 3.4 % of config 5 when compiled in).
+template <int NEQ, int LANES, bool EXT = false>
 struct Group {
   static constexpr int LD = LANES + 1;
   // identity of this lane
@@ -36,18 +39,19 @@ struct Group {
   // and 9.5 % of config 5's time less than the 5-round butterfly of 64-bit shuffles and compares it
   // replaces.  Sub-warp groups keep the butterfly: redux with a partial member mask measured 5 % slower.
   __device__ __forceinline__ unsigned long long gmax(unsigned long long v) const {
-    if (LANES == 32) {
+    if constexpr (LANES == 32) {
       const unsigned hi = (unsigned)(v >> 32), lo = (unsigned)v;
       const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
       const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
       return ((unsigned long long)mh << 32) | (unsigned long long)ml;
-    }
+    } else {
 #pragma unroll
-    for (int s = LANES / 2; s >= 1; s >>= 1) {
-      unsigned long long o = __shfl_xor_sync(gmask, v, s, LANES);
-      v = o > v ? o : v;
+      for (int s = LANES / 2; s >= 1; s >>= 1) {
+        unsigned long long o = __shfl_xor_sync(gmask, v, s, LANES);
+        v = o > v ? o : v;
+      }
+      return v;
     }
-    return v;
   }
   __device__ __forceinline__ int gmin(int v) const {
 #pragma unroll
@@ -86,13 +90,13 @@ struct Group {
     const double t13third = t13 * (1.0 / 3.0);
     const double invT = 1.0 / T;
     const double rho2 = rho * rho;
-    const double lnrho = rexp ? log_(rho) : 0.0;  // lambda_k *= rho^e_k inside the exponent
+    const double lnrho = (EXT && rexp) ? log_(rho) : 0.0;  // lambda_k *= rho^e_k inside the exponent
     for (int k = lig; k < K; k += LANES) {
       const int4 rpk = reinterpret_cast<const int4 *>(rp)[k];
       const int m = rpk.x & 0xff;
       const int r0 = rpk.y & 0xff, r1 = (rpk.y >> 8) & 0xff, r2 = (rpk.y >> 16) & 0xff;
       double arg = fma_(-B[k], t13, fma_(en[k], lnT9, lnA[k]));
-      if (rexp) arg = fma_(rexp[k], lnrho, arg);
+      if (EXT && rexp) arg = fma_(rexp[k], lnrho, arg);
       const double lam = exp_(arg);
       const double pref = (lam * (m == 1 ? 1.0 : (m == 2 ? rho : rho2))) * invsym[k];
       const double y0 = ysh[r0 + 1];
@@ -157,7 +161,7 @@ struct Group {
     // analytic EOS: c_v = 1.5 R (extra + sum_i (1+Z_i) Y_i) + 4 a T^3 / rho, raw Y, i ascending; every lane
     // computes it (uniform code, identical bits); facv replaces the constant fac
     double facv = fac, invcv = 0.0, T2 = 0.0, invrho = 0.0;
-    if (zp1) {
+    if (EXT && zp1) {
       double ysum = eos_extra;
       for (int i = 0; i < N; i++) ysum = fma_(zp1[i], ysh[i + 1], ysum);
       T2 = T * T;
@@ -213,7 +217,7 @@ struct Group {
         jt = jt0;  // summed alongside f above (same k-ascending fma chain)
       }
       sync();  // rows of the species are complete before the T row is written
-      if (zp1) {
+      if (EXT && zp1) {
         // dT/dt = facv s: the row gains -f_T (dc_v/dy_j) / c_v, dc_v/dT = 12 a T^2/rho, dc_v/dY_j = 1.5 R (1+Z_j)
         const double gq = bcast(f, 0) * invcv;
         const double dcv = (lig == 0) ? ((12.0 * ARAD) * T2) * invrho : ((lig <= N) ? (1.5 * RGAS) * zp1[sp] : 0.0);

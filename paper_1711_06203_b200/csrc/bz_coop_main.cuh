@@ -14,7 +14,7 @@ constexpr int COOP_THREADS = 256;
 // slower.  The sub-warp instances fit 128 registers, and two blocks per SM (16 warps instead of 8) ran
 // 9 % faster (config 3 on burn_coop<14,16>) -- when shared memory allows two blocks, which net_create
 // asks the occupancy calculator.
-template <int NEQ, int LANES>
+template <int NEQ, int LANES, bool EXT>
 __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop_kernel(DevNet net, BurnArgs A) {
   extern __shared__ __align__(16) double smem[];
   constexpr int LD = LANES + 1;
@@ -27,15 +27,15 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
   for (int i = threadIdx.x; i < net.nint; i += blockDim.x) s_int[i] = net.itab[i];
   __syncthreads();
 
-  Group<NEQ, LANES> g;
+  Group<NEQ, LANES, EXT> g;
   g.lig = threadIdx.x & (LANES - 1);
   g.gmask = (LANES == 32) ? 0xffffffffu : (((1u << (LANES & 31)) - 1u) << ((threadIdx.x & 31) & ~(LANES - 1)));
   g.N = N; g.n = n; g.K = K; g.fac = net.fac;
   g.inv_n = 1.0 / (double)n;
   g.lnA = s_dbl; g.en = s_dbl + K; g.B = s_dbl + 2 * K; g.Q = s_dbl + 3 * K; g.invsym = s_dbl + 4 * K;
   g.aion = s_dbl + 5 * K; g.sp_dy = s_dbl + 5 * K + N;
-  g.rexp = net.has_rexp ? s_dbl + 5 * K + N + net.nterm : nullptr;
-  g.zp1 = net.eos ? s_dbl + 5 * K + N + net.nterm + (net.has_rexp ? K : 0) : nullptr;
+  g.rexp = (EXT && net.has_rexp) ? s_dbl + 5 * K + N + net.nterm : nullptr;
+  g.zp1 = (EXT && net.eos) ? s_dbl + 5 * K + N + net.nterm + (net.has_rexp ? K : 0) : nullptr;
   g.eos_extra = net.eos_extra;
   g.rp = s_int; g.sp_off = s_int + 4 * K; g.sp_k = g.sp_off + (N + 1);
   g.cl_off = g.sp_k + net.nterm; g.cl_ks = g.cl_off + (N + 1);
@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
         double xin = 0.0;
         ai = 1.0;
         if (lig >= 1 && lig <= N) {  // internal order: lane 0 = T, lane i + 1 = species i
-          xin = A.X[(long long)(lig - 1) * A.nz + z];
+          xin = A.X[(long long)(lig - 1) * A.ld + z];
           ai = g.aion[lig - 1];
         } else if (lig == 0) {
           xin = A.T[z];
@@ -104,14 +104,14 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
         const double y0 = (lig >= 1 && lig <= N) ? xin / ai : xin;
         if (g.has_src) {
           g.src = 0.0;
-          if (lig >= 1 && lig <= N) g.src = A.src_X[(long long)(lig - 1) * A.nz + z] / ai;
+          if (lig >= 1 && lig <= N) g.src = A.src_X[(long long)(lig - 1) * A.ld + z] / ai;
           else if (lig == 0) g.src = A.src_T[z];
         }
         const bool bad = !(rho > 0.0) || !finite_(rho) || (act && !finite_(y0)) || (lig == 0 && !(y0 > 0.0)) ||
                          (g.has_src && !finite_(g.src));
         if (g.gany(bad)) {  // invalid input zone: outputs = inputs; stay in phase 0
           if (lig >= 1 && lig <= N) {
-            A.X_out[(long long)(lig - 1) * A.nz + z] = xin;
+            A.X_out[(long long)(lig - 1) * A.ld + z] = xin;
           } else if (lig == 0) {
             A.T_out[z] = xin;
             A.nsteps[z] = -4;

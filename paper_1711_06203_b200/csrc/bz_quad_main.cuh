@@ -124,12 +124,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
             y[s] = xin[s];
             bad |= !(y[s] > 0.0) || !finite_(y[s]);
           } else if (i < NEQ) {
-            xin[s] = A.X[(long long)(i - 1) * A.nz + z];
+            xin[s] = A.X[(long long)(i - 1) * A.ld + z];
             y[s] = xin[s] / aion[i - 1];
             bad |= !finite_(y[s]);
           }
           if (has_src && i < NEQ) {
-            const double sv = (i == 0) ? A.src_T[z] : A.src_X[(long long)(i - 1) * A.nz + z] / aion[i - 1];
+            const double sv = (i == 0) ? A.src_T[z] : A.src_X[(long long)(i - 1) * A.ld + z] / aion[i - 1];
             m.src(i) = sv;  // own component only: no intra-quad hazard
             bad |= !finite_(sv);
           }
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
               A.T_out[z] = xin[s];
               A.nsteps[z] = -4;
             } else if (i < NEQ)
-              A.X_out[(long long)(i - 1) * A.nz + z] = xin[s];
+              A.X_out[(long long)(i - 1) * A.ld + z] = xin[s];
           }
           BZQ_COUNT(CN_FAIL);
         } else {

@@ -100,11 +100,13 @@ unsigned long long topology_hash(const bz_net_desc *d) {
 struct Variant {
   const char *name;
   int neq, lanes;
-  KernelFn fn;
+  KernelFn fn;      // the plain model
+  KernelFn fn_ext;  // with density exponents and/or the analytic EOS (bz_net_desc.rate_rho_exp, zion)
 };
 
-#define BZ_VARIANT(NEQ, LANES) \
-  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, (KernelFn)bz::burn_coop_kernel<NEQ, LANES> }
+#define BZ_VARIANT(NEQ, LANES)                                                                      \
+  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false>, \
+    (KernelFn)bz::burn_coop_kernel<NEQ, LANES, true> }
 
 const Variant kVariants[] = {
     BZ_VARIANT(3, 4),   BZ_VARIANT(4, 4),   BZ_VARIANT(8, 8),   BZ_VARIANT(14, 16),
@@ -271,6 +273,10 @@ int static_flatten(const bz_net_desc *d, StaticFlat &F) {
 }  // namespace
 
 
+// burn_zones_host: at most this many chunks, of at least this many zones each
+constexpr int HOST_MAX_CHUNKS = 16;
+constexpr int64_t HOST_MIN_CHUNK = 1 << 20;
+
 struct bz_net {
   int N, n, K;
   bz::DevNet dev;
@@ -278,6 +284,7 @@ struct bz_net {
   int *d_int;
   unsigned long long *d_scratch;  // [0] queue head, [1..8] counters
   const Variant *variant;
+  KernelFn coop_fn;  // variant->fn, or variant->fn_ext when the network carries density exponents or an EOS
   int grid, smem_bytes;
   const QuadVariant *quad;  // non-null: a specialised kernel exists for this topology
   int quad_grid;
@@ -289,10 +296,12 @@ struct bz_net {
   int mxstep, mxnef, mxncf;  // bz_set_limits
   int policy;                // bz_set_policy: 0 fresh matrix every attempt, 1 reuse
   int quad_grid_reuse;
-  // staging for burn_zones_host
+  // staging for burn_zones_host, and the copy streams / events of its pipeline
   double *st_in, *st_out;
   int32_t *st_nsteps;
   int64_t st_cap;
+  cudaStream_t s_in, s_out;
+  cudaEvent_t ev_in[HOST_MAX_CHUNKS], ev_done[HOST_MAX_CHUNKS], ev_start, ev_end;
 };
 
 extern "C" {
@@ -317,6 +326,7 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   std::memset(h, 0, sizeof(*h));
   h->N = N; h->n = n; h->K = K;
   h->variant = pick_variant(n);
+  h->coop_fn = (F.has_rexp || F.eos) ? h->variant->fn_ext : h->variant->fn;
   h->mxstep = bz::MXSTEP; h->mxnef = bz::MXNEF; h->mxncf = bz::MXNCF;
 
   // ---- upload --------------------------------------------------------------------------------
@@ -354,9 +364,9 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   if (h->smem_bytes > optin) return fail(BZ_ERR_NOMEM);
   // the attribute belongs to the kernel, not to the handle: always opt in to the device maximum, so
   // that a later handle with smaller tables cannot lower it under an earlier one
-  if (!cuda_ok(cudaFuncSetAttribute((const void *)h->variant->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
+  if (!cuda_ok(cudaFuncSetAttribute((const void *)h->coop_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
     return fail(BZ_ERR_CUDA);
-  if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->variant->fn,
+  if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->coop_fn,
                                                              bz::COOP_THREADS, h->smem_bytes)))
     return fail(BZ_ERR_CUDA);
   if (bps < 1) return fail(BZ_ERR_NOMEM);
@@ -412,6 +422,16 @@ int net_destroy(bz_net *h) {
   if (h->st_in) cudaFree(h->st_in);
   if (h->st_out) cudaFree(h->st_out);
   if (h->st_nsteps) cudaFree(h->st_nsteps);
+  if (h->s_in) {
+    cudaStreamDestroy(h->s_in);
+    if (h->s_out) cudaStreamDestroy(h->s_out);
+    for (int i = 0; i < HOST_MAX_CHUNKS; i++) {
+      if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
+      if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
+    }
+    if (h->ev_start) cudaEventDestroy(h->ev_start);
+    if (h->ev_end) cudaEventDestroy(h->ev_end);
+  }
   delete h;
   return BZ_OK;
 }
@@ -464,23 +484,15 @@ static bool scalars_ok(double dt, double rtol, double atol) {
   return (dt > 0.0) && (rtol > 0.0) && (atol >= 0.0) && std::isfinite(dt) && std::isfinite(rtol) && std::isfinite(atol);
 }
 
-int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
-                   const double *src_T, const double *src_X, double dt, double rtol, double atol,
-                   double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream) {
-  if (!h) return BZ_ERR_NULL;
-  if (nz < 0) return BZ_ERR_SIZE;
-  if (!scalars_ok(dt, rtol, atol)) return BZ_ERR_SCALAR;
-  if (nz == 0) return BZ_OK;
-  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
-  if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
-  if (h->policy == 1 && !use_quad(h)) return BZ_ERR_UNSUPPORTED;  // reuse exists in the specialised kernels only
-  const int drc = check_device(h);
-  if (drc != BZ_OK) return drc;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  BZ_CUDA(cudaMemsetAsync(h->d_scratch, 0, 16 * sizeof(unsigned long long), st));
+// one launch over nz zones whose rows are `ld` doubles apart; reset_counters = false keeps the event
+// counters of the handle running (the later chunks of burn_zones_host)
+static int launch_burn(const bz_net *h, int64_t nz, int64_t ld, const double *rho, const double *T, const double *X,
+                       const double *src_T, const double *src_X, double dt, double rtol, double atol, double *T_out,
+                       double *X_out, int32_t *nsteps, cudaStream_t st, bool reset_counters) {
+  BZ_CUDA(cudaMemsetAsync(h->d_scratch, 0, (reset_counters ? 16 : 1) * sizeof(unsigned long long), st));
   bz::BurnArgs a;
   a.src_T = src_T; a.src_X = src_X;
-  a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
+  a.nz = nz; a.ld = ld; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
   a.mxstep = h->mxstep; a.mxnef = h->mxnef; a.mxncf = h->mxncf;
@@ -504,9 +516,25 @@ int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double 
   const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
   const int grid = (int)(groups_needed < h->grid ? groups_needed : h->grid);
   void *args[] = {(void *)&h->dev, (void *)&a};
-  BZ_CUDA(cudaLaunchKernel((const void *)h->variant->fn, dim3(grid), dim3(bz::COOP_THREADS), args,
+  BZ_CUDA(cudaLaunchKernel((const void *)h->coop_fn, dim3(grid), dim3(bz::COOP_THREADS), args,
                            (size_t)h->smem_bytes, st));
   return BZ_OK;
+}
+
+int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double *T, const double *X,
+                   const double *src_T, const double *src_X, double dt, double rtol, double atol,
+                   double *T_out, double *X_out, int32_t *nsteps, void *cuda_stream) {
+  if (!h) return BZ_ERR_NULL;
+  if (nz < 0) return BZ_ERR_SIZE;
+  if (!scalars_ok(dt, rtol, atol)) return BZ_ERR_SCALAR;
+  if (nz == 0) return BZ_OK;
+  if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
+  if (h->policy == 1 && !use_quad(h)) return BZ_ERR_UNSUPPORTED;  // reuse exists in the specialised kernels only
+  const int drc = check_device(h);
+  if (drc != BZ_OK) return drc;
+  return launch_burn(h, nz, nz, rho, T, X, src_T, src_X, dt, rtol, atol, T_out, X_out, nsteps,
+                     (cudaStream_t)cuda_stream, true);
 }
 
 int bz_get_counters(const bz_net *h, void *cuda_stream, uint64_t out[8]) {
@@ -529,6 +557,7 @@ int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, c
   if (!scalars_ok(dt, rtol, atol)) return BZ_ERR_SCALAR;  // before anything is staged or enqueued
   if (nz == 0) return BZ_OK;
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
+  if (h->policy == 1 && !use_quad(h)) return BZ_ERR_UNSUPPORTED;
   const int drc = check_device(h);
   if (drc != BZ_OK) return drc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -546,16 +575,56 @@ int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, c
     if (!cuda_ok(cudaMalloc(&h->st_nsteps, (size_t)nz * sizeof(int32_t)))) return BZ_ERR_NOMEM;
     h->st_cap = nz;
   }
+  if (!h->s_in) {  // copy streams and events of the pipeline, made once per handle
+    BZ_CUDA(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+    BZ_CUDA(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    for (int i = 0; i < HOST_MAX_CHUNKS; i++) {
+      BZ_CUDA(cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming));
+      BZ_CUDA(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+    }
+    BZ_CUDA(cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming));
+    BZ_CUDA(cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming));
+  }
+  // Pipeline: the zones are burned in chunks; chunk c's inputs travel on a copy stream while chunk c-1
+  // burns on the caller's stream and chunk c-2's results travel back on a second copy stream (zones are
+  // independent, so chunking changes no result; PCIe is full duplex).  Staging is sized for the whole
+  // call, so chunks never share memory and need no further ordering.  One chunk when the copies are
+  // small beside the burn (a chunk must still fill the GPU: >= HOST_MIN_CHUNK zones).
+  int nchunk = (int)(nz / HOST_MIN_CHUNK);
+  if (nchunk < 1) nchunk = 1;
+  if (nchunk > HOST_MAX_CHUNKS) nchunk = HOST_MAX_CHUNKS;
   double *d_rho = h->st_in, *d_T = h->st_in + nz, *d_X = h->st_in + 2 * nz;
   double *d_To = h->st_out, *d_Xo = h->st_out + nz;
-  BZ_CUDA(cudaMemcpyAsync(d_rho, rho, nz * sizeof(double), cudaMemcpyHostToDevice, st));
-  BZ_CUDA(cudaMemcpyAsync(d_T, T, nz * sizeof(double), cudaMemcpyHostToDevice, st));
-  BZ_CUDA(cudaMemcpyAsync(d_X, X, (size_t)N * nz * sizeof(double), cudaMemcpyHostToDevice, st));
-  int rc = burn_zones(h, nz, d_rho, d_T, d_X, dt, rtol, atol, d_To, d_Xo, h->st_nsteps, cuda_stream);
-  if (rc != BZ_OK) return rc;
-  BZ_CUDA(cudaMemcpyAsync(T_out, d_To, nz * sizeof(double), cudaMemcpyDeviceToHost, st));
-  BZ_CUDA(cudaMemcpyAsync(X_out, d_Xo, (size_t)N * nz * sizeof(double), cudaMemcpyDeviceToHost, st));
-  BZ_CUDA(cudaMemcpyAsync(nsteps, h->st_nsteps, nz * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  const size_t pitch = (size_t)nz * sizeof(double);
+  BZ_CUDA(cudaEventRecord(h->ev_start, st));            // the copies start after the caller's earlier work
+  BZ_CUDA(cudaStreamWaitEvent(h->s_in, h->ev_start, 0));
+  BZ_CUDA(cudaStreamWaitEvent(h->s_out, h->ev_start, 0));
+  for (int c = 0; c < nchunk; c++) {
+    const int64_t z0 = nz * c / nchunk, z1 = nz * (c + 1) / nchunk, m = z1 - z0;
+    const size_t w = (size_t)m * sizeof(double);
+    cudaStream_t si = (nchunk == 1) ? st : h->s_in, so = (nchunk == 1) ? st : h->s_out;
+    BZ_CUDA(cudaMemcpyAsync(d_rho + z0, rho + z0, w, cudaMemcpyHostToDevice, si));
+    BZ_CUDA(cudaMemcpyAsync(d_T + z0, T + z0, w, cudaMemcpyHostToDevice, si));
+    BZ_CUDA(cudaMemcpy2DAsync(d_X + z0, pitch, X + z0, pitch, w, (size_t)N, cudaMemcpyHostToDevice, si));
+    if (nchunk > 1) {
+      BZ_CUDA(cudaEventRecord(h->ev_in[c], si));
+      BZ_CUDA(cudaStreamWaitEvent(st, h->ev_in[c], 0));
+    }
+    const int rc = launch_burn(h, m, nz, d_rho + z0, d_T + z0, d_X + z0, nullptr, nullptr, dt, rtol, atol, d_To + z0,
+                               d_Xo + z0, h->st_nsteps + z0, st, c == 0);
+    if (rc != BZ_OK) return rc;
+    if (nchunk > 1) {
+      BZ_CUDA(cudaEventRecord(h->ev_done[c], st));
+      BZ_CUDA(cudaStreamWaitEvent(so, h->ev_done[c], 0));
+    }
+    BZ_CUDA(cudaMemcpyAsync(T_out + z0, d_To + z0, w, cudaMemcpyDeviceToHost, so));
+    BZ_CUDA(cudaMemcpy2DAsync(X_out + z0, pitch, d_Xo + z0, pitch, w, (size_t)N, cudaMemcpyDeviceToHost, so));
+    BZ_CUDA(cudaMemcpyAsync(nsteps + z0, h->st_nsteps + z0, (size_t)m * sizeof(int32_t), cudaMemcpyDeviceToHost, so));
+  }
+  if (nchunk > 1) {  // the caller's stream is done when the last results have arrived
+    BZ_CUDA(cudaEventRecord(h->ev_end, h->s_out));
+    BZ_CUDA(cudaStreamWaitEvent(st, h->ev_end, 0));
+  }
   return BZ_OK;
 }
 
@@ -588,6 +657,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int N = d->nspec, K = d->nreac, n = N + 1;
   const Variant *v = pick_variant(n);
+  const KernelFn vfn = (F.has_rexp || F.eos) ? v->fn_ext : v->fn;
   const int L = v->lanes;
   const int gpb = bz::COOP_THREADS / L;
   const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
@@ -595,9 +665,9 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   const int smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
   if (smem_bytes > sd->smem_optin) return BZ_ERR_NOMEM;
   // opt in to the device's maximum: never lowers what a handle of net_create has set for this kernel
-  BZ_CUDA(cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, sd->smem_optin));
+  BZ_CUDA(cudaFuncSetAttribute((const void *)vfn, cudaFuncAttributeMaxDynamicSharedMemorySize, sd->smem_optin));
   int bps = 0;
-  BZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)v->fn, bz::COOP_THREADS, smem_bytes));
+  BZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)vfn, bz::COOP_THREADS, smem_bytes));
   if (bps < 1) return BZ_ERR_NOMEM;
 
   unsigned char *base = sd->ptr;
@@ -617,7 +687,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   dn.has_rexp = F.has_rexp;
   bz::BurnArgs a;
   a.src_T = nullptr; a.src_X = nullptr;
-  a.nz = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
+  a.nz = nz; a.ld = nz; a.rho = rho; a.T = T; a.X = X; a.dt = dt; a.rtol = rtol; a.atol = atol;
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = reinterpret_cast<unsigned long long *>(base);
   a.counters = reinterpret_cast<unsigned long long *>(base) + 1;
@@ -627,7 +697,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   const long long full = (long long)sd->sms * bps;
   const int grid = (int)(groups_needed < full ? groups_needed : full);
   void *args[] = {(void *)&dn, (void *)&a};
-  BZ_CUDA(cudaLaunchKernel((const void *)v->fn, dim3(grid), dim3(bz::COOP_THREADS), args, (size_t)smem_bytes, st));
+  BZ_CUDA(cudaLaunchKernel((const void *)vfn, dim3(grid), dim3(bz::COOP_THREADS), args, (size_t)smem_bytes, st));
   return BZ_OK;
 }
 

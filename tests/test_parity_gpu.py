@@ -149,6 +149,37 @@ def test_host_path_matches_device_path():
 # one burn_zones call), compared on sampled zones the oracle computes one by one, plus properties
 # that hold at any size (mass invariant, valid step counts, finite outputs).
 # ---------------------------------------------------------------------------------------------
+def test_host_path_pipeline_in_chunks():
+    """burn_zones_host pipelines batches of >= 2^21 zones in chunks over two copy streams: same results
+    as the device path bit for bit, counters = totals over the chunks, and the caller's stream is
+    complete only when the last result has arrived (the outputs are read right after one synchronise)."""
+    import torch
+    import paper_1711_06203_b200 as bz
+    w = make_workload(4, zones=np.arange(0, 256 ** 3, 5))          # 3 355 444 zones -> 3 chunks
+    assert w.nz > 3 * (1 << 20)
+    dev = torch.device("cuda:0")
+    net = bz.net_create(w.net)
+    To, Xo, ns = bz.burn_zones(net, torch.from_numpy(w.rho).to(dev), torch.from_numpy(w.T).to(dev),
+                               torch.from_numpy(w.X).to(dev), w.dt, w.rtol, w.atol)
+    torch.cuda.synchronize()
+    cnt_dev = bz.get_counters(net)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    Th = torch.full((w.nz,), -1.0, dtype=torch.float64).pin_memory()
+    Xh = torch.full((w.net.nspec, w.nz), -1.0, dtype=torch.float64).pin_memory()
+    nh = torch.full((w.nz,), -99, dtype=torch.int32).pin_memory()
+    side = torch.cuda.Stream()
+    for _ in range(2):                                             # twice: the pipeline's events are reused
+        Th.fill_(-1.0), Xh.fill_(-1.0), nh.fill_(-99)
+        with torch.cuda.stream(side):
+            bz.burn_zones_host(net, pin(w.rho), pin(w.T), pin(w.X), w.dt, w.rtol, w.atol, Th, Xh, nh, stream=side)
+        side.synchronize()                                         # ONLY the caller's stream
+        assert np.array_equal(nh.numpy(), ns.cpu().numpy())
+        assert np.array_equal(Th.numpy(), To.cpu().numpy()) and np.array_equal(Xh.numpy(), Xo.cpu().numpy())
+        assert bz.get_counters(net, stream=side) == cnt_dev
+    assert ns.cpu().numpy().max() > 100
+    bz.net_destroy(net)
+
+
 def _full_size_check(config, sample_idx, scale=None):
     import torch
     import paper_1711_06203_b200 as bz
