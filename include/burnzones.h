@@ -123,11 +123,12 @@ int burn_zones_src(const bz_net *net, int64_t nz, const double *rho, const doubl
 /* The same burn with HOST arrays (pinned memory recommended): copies inputs to library-owned device
  * staging, burns, copies the three outputs back, and returns without synchronising; everything is
  * ordered after the earlier work of `cuda_stream`, and `cuda_stream` is complete only when the last
- * result has arrived.  Batches of >= 2^21 zones are PIPELINED in up to 16 chunks: chunk c's inputs
- * travel on a library-owned copy stream while chunk c-1 burns on `cuda_stream` and chunk c-2's
- * results travel back on a second copy stream (zones are independent: the results are those of
- * burn_zones; bz_get_counters returns the totals over all chunks).  This is the end-to-end path
- * bench.py times. */
+ * result has arrived.  Batches of >= 2^23 zones are PIPELINED in chunks of >= 2^22 zones (at most 8):
+ * chunk c's inputs travel on a library-owned copy stream while chunk c-1 burns on `cuda_stream` and
+ * chunk c-2's results travel back on a second copy stream (zones are independent: the results are
+ * those of burn_zones; bz_get_counters returns the totals over all chunks).  Chunks are large on
+ * purpose: each is its own launch and pays the serial tail of its slowest zone.  This is the
+ * end-to-end path bench.py times. */
 int burn_zones_host(bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
                     double dt, double rtol, double atol, double *T_out, double *X_out,
                     int32_t *nsteps, void *cuda_stream);

@@ -88,6 +88,35 @@ __device__ __forceinline__ double eta_of(double E, double bias, int p) {
   return 1.0 / (root + ADDON);
 }
 
+// C.2-D, the decision proper, shared by both kernels: the next step-size ratio eta and the order action
+// (-1 lower, 0 keep, +1 raise) from the three candidate etas.  order_due: the order may change at this
+// step (nqwait reached 0); otherwise only eta_q counts.  Then THRESH and the growth cap.
+__device__ __forceinline__ void select_eta(bool order_due, double etaq, double etaqm1, double etaqp1, double etamax,
+                                           double &eta, int &action) {
+  eta = etaq;
+  action = 0;
+  if (order_due) {
+    if (etaq >= etaqp1) {
+      if (!(etaq >= etaqm1)) {
+        eta = etaqm1;
+        action = -1;
+      }
+    } else if (etaqp1 > etaqm1) {
+      eta = etaqp1;
+      action = +1;
+    } else {
+      eta = etaqm1;
+      action = -1;
+    }
+  }
+  if (eta < THRESH) {
+    eta = 1.0;
+    action = 0;
+  } else if (eta > etamax) {
+    eta = etamax;
+  }
+}
+
 template <int NEQ, int LANES>
 struct CoopSmem {
   // per-group scratch, in doubles

@@ -273,9 +273,13 @@ int static_flatten(const bz_net_desc *d, StaticFlat &F) {
 }  // namespace
 
 
-// burn_zones_host: at most this many chunks, of at least this many zones each
-constexpr int HOST_MAX_CHUNKS = 16;
-constexpr int64_t HOST_MIN_CHUNK = 1 << 20;
+// burn_zones_host: at most this many chunks, of at least this many zones each.  Every chunk is its own
+// persistent launch and pays its own serial tail (a zone of 400 steps is ~8 ms of dependent attempts
+// however few zones the launch has), so small chunks cost more than their copies hide: measured on
+// config 4 (16.8 M zones, 78 ms burn, 2 x 31 ms copies): 1 chunk 150 ms, 2 chunks 116, 4 chunks 103.5,
+// 16 chunks 146.
+constexpr int HOST_MAX_CHUNKS = 8;
+constexpr int64_t HOST_MIN_CHUNK = 1 << 22;
 
 struct bz_net {
   int N, n, K;
@@ -588,8 +592,8 @@ int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, c
   // Pipeline: the zones are burned in chunks; chunk c's inputs travel on a copy stream while chunk c-1
   // burns on the caller's stream and chunk c-2's results travel back on a second copy stream (zones are
   // independent, so chunking changes no result; PCIe is full duplex).  Staging is sized for the whole
-  // call, so chunks never share memory and need no further ordering.  One chunk when the copies are
-  // small beside the burn (a chunk must still fill the GPU: >= HOST_MIN_CHUNK zones).
+  // call, so chunks never share memory and need no further ordering.  Batches below 2 x HOST_MIN_CHUNK
+  // zones go in one piece on the caller's stream.
   int nchunk = (int)(nz / HOST_MIN_CHUNK);
   if (nchunk < 1) nchunk = 1;
   if (nchunk > HOST_MAX_CHUNKS) nchunk = HOST_MAX_CHUNKS;
