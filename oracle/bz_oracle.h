@@ -25,9 +25,14 @@
  *   of the accepted values (variable steps); failure codes -1 (real inputs), -2, -3 (limits as
  *   parameters).  Each of these pins was checked to turn red under a perturbation of the line it
  *   covers (commit message of the pins).
+ *   Model extensions: density exponents (closed form in rho, tests/test_urca9_like.py), analytic EOS
+ *   (exact energy integral, tests/test_eos_cv.py), policy 1 (tests/test_oracle_reuse.py): pinned; 11 of
+ *   12 perturbations of their lines turn a pin red.
  *   PARITY UNPINNED: only the VALUES of the heuristics constants (BIAS1..3, THRESH, ETAMAX, ETAMIN,
- *   ETAMXF, ETACF, NTOL, CRDOWN, RDIV, ADDON, SLIVER, the default limits) -- any values pass the
- *   pins; they are fixed by DESIGN.md section 3 only.
+ *   ETAMXF, ETACF, NTOL, CRDOWN, RDIV, ADDON, SLIVER, the default limits; under policy 1 also CCMAX's
+ *   value and the 2/(1 + gamma/gamma_P) scale of a stale solve, which moves the Newton iteration's path
+ *   but not the corrector solution it converges to) -- any values pass the pins; they are fixed by
+ *   DESIGN.md sections 3 and 12 only.
  */
 #ifndef BZ_ORACLE_H
 #define BZ_ORACLE_H
