@@ -41,8 +41,8 @@ typedef enum {
   BZ_ERR_SCALAR = -4,  /* dt <= 0, rtol <= 0, atol < 0, or non-finite                         */
   BZ_ERR_CUDA = -5,    /* CUDA runtime error; the cudaError_t is in bz_last_cuda_error()      */
   BZ_ERR_NOMEM = -6,   /* host or device allocation failed                                    */
-  BZ_ERR_UNSUPPORTED = -7, /* the selected kernel cannot do what was asked (bz_set_policy 1 on the
-                              generic cooperative kernel)                                          */
+  BZ_ERR_UNSUPPORTED = -7, /* the combination has no kernel (bz_set_policy 1 on a network with density
+                              exponents or an EOS)                                                 */
   BZ_ERR_DEVICE = -8   /* the handle was created on another device than the current one        */
 } bz_status;
 
@@ -193,8 +193,9 @@ int bz_set_schedule(bz_net *net, int kind);
  *          configs at the same step count.  Results are bit-identical to the oracle's policy 1 (not
  *          to policy 0: the two differ at the level of the integration tolerance).  Validated on the
  *          smooth networks (configs 1-4); on config 5 it loses accuracy on trace species.
- * Served by the network-specialised kernels only: with kind 1, burn_zones on a network that runs on
- * the generic cooperative kernel returns BZ_ERR_UNSUPPORTED. */
+ * Served by both kernels for the plain model; a network that carries density exponents or an EOS
+ * (rate_rho_exp, zion) has no kept-matrix instantiation: burn_zones then returns BZ_ERR_UNSUPPORTED.
+ * burn_zones_static always uses kind 0. */
 int bz_set_policy(bz_net *net, int kind);
 
 /* Limits behind the per-zone failure codes: accepted steps (-3), error-test failures on one step

@@ -14,7 +14,10 @@ constexpr int COOP_THREADS = 256;
 // slower.  The sub-warp instances fit 128 registers, and two blocks per SM (16 warps instead of 8) ran
 // 9 % faster (config 3 on burn_coop<14,16>) -- when shared memory allows two blocks, which net_create
 // asks the occupancy calculator.
-template <int NEQ, int LANES, bool EXT>
+// REUSE: the Newton-matrix policy of bz_set_policy(net, 1), a separate instantiation.  A
+// group owns its zone's factors (LuRow, registers) and nothing of them is shared across groups, so a
+// group that keeps its matrix simply skips Jacobian and LU: no warp-level sharing as in the quad kernel.
+template <int NEQ, int LANES, bool EXT, bool REUSE>
 __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop_kernel(DevNet net, BurnArgs A) {
   extern __shared__ __align__(16) double smem[];
   constexpr int LD = LANES + 1;
@@ -70,6 +73,10 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
   double h = 0.0, t = 0.0, etamax = ETAMX1, hS = 0.0;
   int q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0, ncf = 0, nef = 0;
   bool newstep = true, last = false;
+  // REUSE: gamma_P and the step count of the kept factorisation; a factorisation exists; a failure asked for a fresh one
+  double gamP = 0.0;
+  int nslp = 0;
+  bool haveP = false, forceP = false;
   double tau[QMAX + 1];
 #pragma unroll
   for (int i = 0; i <= QMAX; i++) tau[i] = 0.0, Z[i] = 0.0;
@@ -142,6 +149,7 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
           Z[1] = h * f;
           q = 1, nqwait = 2, qS = 0, nst = 0, ntau = 0;
           t = 0.0, etamax = ETAMX1, hS = 0.0, S = 0.0;
+          if (REUSE) gamP = 0.0, nslp = 0, haveP = false, forceP = false;
 #pragma unroll
           for (int i = 0; i <= QMAX; i++) tau[i] = 0.0;
           newstep = true;

@@ -100,13 +100,15 @@ unsigned long long topology_hash(const bz_net_desc *d) {
 struct Variant {
   const char *name;
   int neq, lanes;
-  KernelFn fn;      // the plain model
-  KernelFn fn_ext;  // with density exponents and/or the analytic EOS (bz_net_desc.rate_rho_exp, zion)
+  KernelFn fn;        // the plain model
+  KernelFn fn_ext;    // with density exponents and/or the analytic EOS (bz_net_desc.rate_rho_exp, zion)
+  KernelFn fn_reuse;  // the plain model under bz_set_policy 1 (kept Newton matrix)
 };
 
-#define BZ_VARIANT(NEQ, LANES)                                                                      \
-  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false>, \
-    (KernelFn)bz::burn_coop_kernel<NEQ, LANES, true> }
+#define BZ_VARIANT(NEQ, LANES)                                                                             \
+  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false, false>, \
+    (KernelFn)bz::burn_coop_kernel<NEQ, LANES, true, false>,                                               \
+    (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false, true> }
 
 const Variant kVariants[] = {
     BZ_VARIANT(3, 4),   BZ_VARIANT(4, 4),   BZ_VARIANT(8, 8),   BZ_VARIANT(14, 16),
@@ -289,7 +291,8 @@ struct bz_net {
   unsigned long long *d_scratch;  // [0] queue head, [1..8] counters
   const Variant *variant;
   KernelFn coop_fn;  // variant->fn, or variant->fn_ext when the network carries density exponents or an EOS
-  int grid, smem_bytes;
+  bool ext;          // ... which also means: no reuse policy on the cooperative kernel for this network
+  int grid, grid_reuse, smem_bytes;
   const QuadVariant *quad;  // non-null: a specialised kernel exists for this topology
   int quad_grid;
   double *d_quad_coef, *d_quad_scratch;
@@ -330,7 +333,8 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   std::memset(h, 0, sizeof(*h));
   h->N = N; h->n = n; h->K = K;
   h->variant = pick_variant(n);
-  h->coop_fn = (F.has_rexp || F.eos) ? h->variant->fn_ext : h->variant->fn;
+  h->ext = (F.has_rexp || F.eos);
+  h->coop_fn = h->ext ? h->variant->fn_ext : h->variant->fn;
   h->mxstep = bz::MXSTEP; h->mxnef = bz::MXNEF; h->mxncf = bz::MXNCF;
 
   // ---- upload --------------------------------------------------------------------------------
@@ -375,6 +379,13 @@ int net_create(const bz_net_desc *d, bz_net **out) {
     return fail(BZ_ERR_CUDA);
   if (bps < 1) return fail(BZ_ERR_NOMEM);
   h->grid = sms * bps;
+  if (!cuda_ok(cudaFuncSetAttribute((const void *)h->variant->fn_reuse, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
+    return fail(BZ_ERR_CUDA);
+  if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->variant->fn_reuse,
+                                                             bz::COOP_THREADS, h->smem_bytes)))
+    return fail(BZ_ERR_CUDA);
+  if (bps < 1) return fail(BZ_ERR_NOMEM);
+  h->grid_reuse = sms * bps;
 
   // ---- network-specialised quad kernel for known topologies ---------------------------------------
   const unsigned long long th = topology_hash(d);
@@ -518,10 +529,11 @@ static int launch_burn(const bz_net *h, int64_t nz, int64_t ld, const double *rh
   }
   const int L = h->variant->lanes;
   const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
-  const int grid = (int)(groups_needed < h->grid ? groups_needed : h->grid);
+  const int cfull = h->policy == 1 ? h->grid_reuse : h->grid;
+  const int grid = (int)(groups_needed < cfull ? groups_needed : cfull);
+  const KernelFn cfn = h->policy == 1 ? h->variant->fn_reuse : h->coop_fn;
   void *args[] = {(void *)&h->dev, (void *)&a};
-  BZ_CUDA(cudaLaunchKernel((const void *)h->coop_fn, dim3(grid), dim3(bz::COOP_THREADS), args,
-                           (size_t)h->smem_bytes, st));
+  BZ_CUDA(cudaLaunchKernel((const void *)cfn, dim3(grid), dim3(bz::COOP_THREADS), args, (size_t)h->smem_bytes, st));
   return BZ_OK;
 }
 
@@ -534,7 +546,7 @@ int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double 
   if (nz == 0) return BZ_OK;
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
   if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
-  if (h->policy == 1 && !use_quad(h)) return BZ_ERR_UNSUPPORTED;  // reuse exists in the specialised kernels only
+  if (h->policy == 1 && h->ext) return BZ_ERR_UNSUPPORTED;  // no kept-matrix instantiation with exponents / EOS
   const int drc = check_device(h);
   if (drc != BZ_OK) return drc;
   return launch_burn(h, nz, nz, rho, T, X, src_T, src_X, dt, rtol, atol, T_out, X_out, nsteps,
@@ -561,7 +573,7 @@ int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, c
   if (!scalars_ok(dt, rtol, atol)) return BZ_ERR_SCALAR;  // before anything is staged or enqueued
   if (nz == 0) return BZ_OK;
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
-  if (h->policy == 1 && !use_quad(h)) return BZ_ERR_UNSUPPORTED;
+  if (h->policy == 1 && h->ext) return BZ_ERR_UNSUPPORTED;
   const int drc = check_device(h);
   if (drc != BZ_OK) return drc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -661,7 +673,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int N = d->nspec, K = d->nreac, n = N + 1;
   const Variant *v = pick_variant(n);
-  const KernelFn vfn = (F.has_rexp || F.eos) ? v->fn_ext : v->fn;
+  const KernelFn vfn = (F.has_rexp || F.eos) ? v->fn_ext : v->fn;  // (policy 0 only)
   const int L = v->lanes;
   const int gpb = bz::COOP_THREADS / L;
   const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;

@@ -170,14 +170,15 @@ def test_static_schedule_gives_the_same_bits(kind):
 # ---------------------------------------------------------------------------------------------
 # Newton-matrix reuse (bz_set_policy 1, "BZ-BDF v2"): bit-identical to the oracle's policy 1
 # ---------------------------------------------------------------------------------------------
-def _burn_v2(net_d, rho, T, X, dt, rtol, atol, src=None):
+def _burn_v2(net_d, rho, T, X, dt, rtol, atol, src=None, kind="auto"):
     import torch
     import paper_1711_06203_b200 as bz
     dev = torch.device("cuda:0")
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     net = bz.net_create(net_d)
+    net.select_kernel(kind)
     net.set_policy("reuse")
-    assert net.kernel_name.startswith("burn_quad")
+    assert net.kernel_name.startswith("burn_quad" if kind == "auto" else "burn_coop")
     if src is None:
         To, Xo, ns = bz.burn_zones(net, d(rho), d(T), d(X), dt, rtol, atol)
     else:
@@ -239,10 +240,37 @@ def test_reuse_policy_hard_inputs():
     _same(gpu, (ref[0], ref[1], ref[2], cr))
 
 
-def test_reuse_policy_needs_a_specialised_kernel():
+@pytest.mark.parametrize("case", ["config3", "config2", "config5", "aprox13like", "stress"])
+def test_reuse_policy_on_the_cooperative_kernel(case):
+    """The generic kernel's kept-matrix instantiation: a group owns its zone's factors, so a group that
+    keeps its matrix simply skips Jacobian and LU.  Bit-identical to the oracle's policy 1 (on config 5
+    too: parity does not depend on how accurate the policy is there)."""
+    from workloads import make_aprox13_like_workload
+    if case == "config3":
+        w = make_workload(3, zones=509)
+    elif case == "config2":
+        w = make_workload(2, zones=61)
+    elif case == "config5":
+        w = make_workload(5, zones=4099)
+    elif case == "aprox13like":
+        w = make_aprox13_like_workload(1024)
+    else:
+        net_d, rho, T, X, dt = _stress_zones(3, nz=512)
+        w = make_workload(3, zones=[0])
+        w.rho, w.T, w.X, w.dt = rho, T, X, dt
+    gpu = _burn_v2(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, kind="coop")
+    ref = oracle.burn(w.net, w.rho, w.T, w.X, w.dt, w.rtol, w.atol, norm_lanes=gpu[4], policy=1)
+    cr = {k: v for k, v in ref[3].items() if k != "nstale"}
+    _same(gpu, (ref[0], ref[1], ref[2], cr))
+    assert gpu[3]["nlu"] < 0.3 * gpu[3]["nst"] + w.nz
+    _record(f"reuse_coop:{case}", dict(kernel=gpu[5], nst=gpu[3]["nst"], nlu=gpu[3]["nlu"], nstale=ref[3]["nstale"]))
+
+
+def test_reuse_policy_has_no_instantiation_with_extensions():
     import torch
     import paper_1711_06203_b200 as bz
-    w = make_workload(5, zones=65521)
+    from workloads import make_urca9_like_workload
+    w = make_urca9_like_workload(64)
     dev = torch.device("cuda:0")
     net = bz.net_create(w.net)
     net.set_policy("reuse")
@@ -250,4 +278,8 @@ def test_reuse_policy_needs_a_specialised_kernel():
         bz.burn_zones(net, torch.from_numpy(w.rho).to(dev), torch.from_numpy(w.T).to(dev), torch.from_numpy(w.X).to(dev),
                       w.dt, w.rtol, w.atol)
     assert e.value.code == -7
+    net.set_policy("fresh")
+    bz.burn_zones(net, torch.from_numpy(w.rho).to(dev), torch.from_numpy(w.T).to(dev), torch.from_numpy(w.X).to(dev),
+                  w.dt, w.rtol, w.atol)
+    torch.cuda.synchronize()
     bz.net_destroy(net)
