@@ -283,3 +283,43 @@ def test_reuse_policy_has_no_instantiation_with_extensions():
                   w.dt, w.rtol, w.atol)
     torch.cuda.synchronize()
     bz.net_destroy(net)
+
+
+# ---------------------------------------------------------------------------------------------
+# Fuzz: random networks of random sizes through every instantiation of the generic kernel
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(12))
+def test_fuzz_generic_kernel_instantiations(seed):
+    """nspec in 1..31 (all seven lane/size instances, padded ones included), random topology, and per seed
+    one of: plain model, density exponents, EOS, both, plain model under the kept-matrix policy.  Bit-exact."""
+    import torch
+    import paper_1711_06203_b200 as bz
+    from test_parity_gpu import _random_network
+    rng = np.random.default_rng(7000 + seed)
+    nspec = int([2, 3, 4, 7, 8, 11, 15, 16, 22, 30, 31, 6][seed])
+    nreac = int(rng.integers(nspec, 4 * nspec + 1))
+    net_d = _random_network(nspec, nreac, seed=8000 + seed)
+    mode = ["plain", "rexp", "eos", "both", "reuse", "plain", "reuse", "eos", "rexp", "both", "reuse", "plain"][seed]
+    if mode in ("rexp", "both"):
+        net_d.rate_rho_exp = np.where(rng.random(nreac) < 0.4, rng.uniform(-0.5, 0.5, nreac), 0.0)
+    if mode in ("eos", "both"):
+        net_d.zion = np.round(net_d.aion / 2)
+        net_d.eos_extra = 0.002
+    nz = 96
+    rho = 10 ** rng.uniform(4, 7, nz)
+    T = rng.uniform(8e8, 3e9, nz)
+    X = rng.random((nspec, nz)) + 0.01
+    X /= X.sum(axis=0)
+    dev = torch.device("cuda:0")
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    net = bz.net_create(net_d)
+    pol = 1 if mode == "reuse" else 0
+    net.set_policy("reuse" if pol else "fresh")
+    assert net.kernel_name.startswith("burn_coop")
+    To, Xo, ns = bz.burn_zones(net, d(rho), d(T), d(X), 1e-6, 1e-8, 1e-12)
+    torch.cuda.synchronize()
+    cnt = bz.get_counters(net)
+    ref = oracle.burn(net_d, rho, T, X, 1e-6, 1e-8, 1e-12, norm_lanes=net.norm_lanes, policy=pol)
+    cr = {k: v for k, v in ref[3].items() if k != "nstale"}
+    _same((To.cpu().numpy(), Xo.cpu().numpy(), ns.cpu().numpy(), cnt), (ref[0], ref[1], ref[2], cr))
+    bz.net_destroy(net)
