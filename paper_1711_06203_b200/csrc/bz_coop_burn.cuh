@@ -14,6 +14,16 @@ struct LuRow {
 
   __device__ __forceinline__ int pivot_lane(int k) const { return (plpack[k >> 2] >> ((k & 3) * 8)) & 0xff; }
 
+  // my row of P = I - gamma*J, from the row of J that the rates left in the group's matrix M
+  template <class G>
+  __device__ __forceinline__ void form(const G &g, double gamma, bool act, int n) {
+#pragma unroll
+    for (int j = 0; j < NEQ; j++) {
+      const double Jij = (act && j < n) ? g.M[g.lig * (LANES + 1) + j] : 0.0;
+      a[j] = fma_(-gamma, Jij, (j == g.lig) ? 1.0 : 0.0);
+    }
+  }
+
   // a5: in-place LU with partial pivoting, LINPACK tie-break (first maximal |a_ik| in the
   // current row order), rows never move.  Returns false if a pivot column is all zero.
   template <class G>
@@ -82,6 +92,106 @@ struct LuRow {
     g.sync();
     return (g.lig < NEQ) ? g.xs[g.lig] : 0.0;
   }
+};
+
+// The same factorisation with the rows left where the rates put them: in the group's shared-memory
+// matrix M (lane i owns row i at M + i*LD, LD = LANES + 1: lanes i and i + 16 share a bank, the minimum
+// for 64-bit accesses).  A warp-per-zone lane then carries no row in registers (62 of them for n = 31),
+// the pivot row is read where it lies instead of being published to a broadcast buffer, and the loops
+// over k and j are rolled: the factorisation is 2 KB of code instead of 54 KB.  Operations and their
+// order are those of LuRow: same bits.  The pivot lanes of the steps are kept in the group's old
+// broadcast buffer (urow) as ints.
+template <int NEQ, int LANES>
+struct LuSmem {
+  static constexpr int LD = LANES + 1;
+  double myinv;  // 1/pivot of the step at which my row was the pivot row
+  int pos;       // LINPACK position of my row
+
+  template <class G>
+  __device__ __forceinline__ void form(const G &g, double gamma, bool act, int n) {
+    if (g.lig < NEQ) {
+      double *row = g.M + g.lig * LD;
+#pragma unroll 4
+      for (int j = 0; j < NEQ; j++) {
+        const double Jij = (act && j < n) ? row[j] : 0.0;
+        row[j] = fma_(-gamma, Jij, (j == g.lig) ? 1.0 : 0.0);
+      }
+    }
+  }
+
+  template <class G>
+  __device__ __forceinline__ bool factor(const G &g) {
+    const int lig = g.lig;
+    pos = lig;
+    myinv = 0.0;
+    bool ok = true;
+    double *row = g.M + (lig < NEQ ? lig : 0) * LD;
+    int *pls = reinterpret_cast<int *>(g.urow);
+#pragma unroll 1
+    for (int k = 0; k < NEQ; k++) {
+      g.sync();  // the rows as updated in step k - 1 (or formed) are visible to every lane
+      const double my = row[k];
+      const bool cand0 = (pos >= k) && (lig < NEQ);
+      const unsigned long long key =
+          cand0 ? (unsigned long long)(__double_as_longlong(my) & 0x7fffffffffffffffLL) : 0ull;
+      const unsigned long long kmax = g.gmax(key);
+      if (kmax == 0ull || kmax > 0x7ff0000000000000ull) ok = false;  // zero or NaN pivot column
+      const bool cand = cand0 && (key == kmax);
+      unsigned ball = g.gballot(cand);
+      if (__popc(ball) > 1) {  // exact tie: smallest LINPACK position wins
+        const int mp = g.gmin(cand ? pos : 0x7fffffff);
+        ball = g.gballot(cand && pos == mp);
+      }
+      const int pl = __ffs(ball) - 1;
+      if (lig == 0) pls[k] = pl;
+      const int ppos = __shfl_sync(g.gmask, pos, pl & (LANES - 1), LANES);
+      const bool isp = (lig == pl);
+      if (pos == k) pos = ppos;
+      if (isp) pos = k;
+      const double *prow = g.M + (pl & (LANES - 1)) * LD;  // the pivot row, where it lies (its owner does not touch it now)
+      const double inv = 1.0 / prow[k];
+      if (isp) myinv = inv;
+      if (pos > k && lig < NEQ) {
+        const double l = my * inv;
+        row[k] = l;
+#pragma unroll 4
+        for (int j = k + 1; j < NEQ; j++) row[j] = fma_(-l, prow[j], row[j]);
+      }
+    }
+    g.sync();
+    return ok;
+  }
+
+  template <class G>
+  __device__ __forceinline__ double solve(const G &g, double b) const {
+    const double *row = g.M + (g.lig < NEQ ? g.lig : 0) * LD;
+    const int *pls = reinterpret_cast<const int *>(g.urow);
+#pragma unroll
+    for (int k = 0; k < NEQ; k++) {
+      const double bk = g.bcast(b, pls[k]);
+      if (pos > k) b = fma_(-row[k], bk, b);
+    }
+#pragma unroll
+    for (int k = NEQ - 1; k >= 0; k--) {
+      const double x = b * myinv;
+      if (pos == k) b = x;
+      const double xk = g.bcast(x, pls[k]);
+      if (pos < k) b = fma_(-row[k], xk, b);
+    }
+    g.sync();
+    if (g.lig < NEQ) g.xs[pos] = b;
+    g.sync();
+    return (g.lig < NEQ) ? g.xs[g.lig] : 0.0;
+  }
+};
+
+template <int NEQ, int LANES, bool SMEM = (LANES == 32)>
+struct LuPick {
+  typedef LuRow<NEQ, LANES> type;
+};
+template <int NEQ, int LANES>
+struct LuPick<NEQ, LANES, true> {
+  typedef LuSmem<NEQ, LANES> type;
 };
 
 // Nordsieck helpers on my component.  Arrays are indexed with compile-time indices only.

@@ -9,6 +9,17 @@
 namespace bz {
 
 constexpr int COOP_THREADS = 256;
+// Threads per block of an instance.  The warp-per-zone instances factorise in place in the group's
+// shared-memory matrix (LuSmem, bz_coop_burn.cuh), which takes the 31-entry row out of every lane's
+// registers: 128 registers instead of 255, so one block holds 16 zones (16 warps) instead of 8.  Measured on
+// config 5 (131 072-zone sample): rows in registers, 256 threads 3 447 ms; rows in shared memory, 256
+// threads 4 290 ms (two loads and a store per FMA), 384 threads 3 415 ms, 512 threads 3 258 ms.  net_create
+// launches fewer threads when the tables of a large network leave no room for 16 groups.
+template <int LANES>
+struct CoopShape {
+  static constexpr int THREADS = (LANES == 32) ? 512 : COOP_THREADS;
+  static constexpr int MINB = (LANES == 32) ? 1 : 2;
+};
 // Blocks per SM: the warp-per-zone instances (LANES == 32: a row of up to 32 doubles per lane) need the
 // full 255 registers, one block per SM; with 128 registers they spill 1.7 KB per thread and ran 28 %
 // slower.  The sub-warp instances fit 128 registers, and two blocks per SM (16 warps instead of 8) ran
@@ -18,7 +29,7 @@ constexpr int COOP_THREADS = 256;
 // group owns its zone's factors (LuRow, registers) and nothing of them is shared across groups, so a
 // group that keeps its matrix simply skips Jacobian and LU: no warp-level sharing as in the quad kernel.
 template <int NEQ, int LANES, bool EXT, bool REUSE>
-__global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop_kernel(DevNet net, BurnArgs A) {
+__global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::MINB) burn_coop_kernel(DevNet net, BurnArgs A) {
   extern __shared__ __align__(16) double smem[];
   constexpr int LD = LANES + 1;
   const int N = net.N, n = net.n, K = net.K;
@@ -62,7 +73,8 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
   const double dt = A.dt, rtol = A.rtol, atol = A.atol;
   unsigned long long c_nst = 0, c_rhs = 0, c_jac = 0, c_lu = 0, c_sol = 0, c_etf = 0, c_cfn = 0, c_fail = 0;
 
-  LuRow<NEQ, LANES> lu;
+  // warp-per-zone instances factorise in place in shared memory, sub-warp instances in registers
+  typename LuPick<NEQ, LANES>::type lu;
 
   // per-zone integrator state, persistent across loop trips (registers; uniform within the group
   // except the per-component Z, w, S)
@@ -88,8 +100,8 @@ __global__ void __launch_bounds__(COOP_THREADS, (LANES == 32 ? 1 : 2)) burn_coop
       // (bz_set_schedule(1) switches a2 off for the before/after measurement: group g then burns zones
       // g, g + G, g + 2G, ... with G = groups of the grid; results are the same, only the balance differs)
       if (A.static_sched) {
-        const long long G = (long long)gridDim.x * (COOP_THREADS / LANES);
-        z = started ? z + G : (long long)blockIdx.x * (COOP_THREADS / LANES) + threadIdx.x / LANES;
+        const long long G = (long long)gridDim.x * (blockDim.x / LANES);
+        z = started ? z + G : (long long)blockIdx.x * (blockDim.x / LANES) + threadIdx.x / LANES;
         started = true;
       } else {
         if (lig == 0) z = (long long)atomicAdd(A.queue, 1ull);

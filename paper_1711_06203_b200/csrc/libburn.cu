@@ -99,14 +99,15 @@ unsigned long long topology_hash(const bz_net_desc *d) {
 
 struct Variant {
   const char *name;
-  int neq, lanes;
+  int neq, lanes, threads;
   KernelFn fn;        // the plain model
   KernelFn fn_ext;    // with density exponents and/or the analytic EOS (bz_net_desc.rate_rho_exp, zion)
   KernelFn fn_reuse;  // the plain model under bz_set_policy 1 (kept Newton matrix)
 };
 
 #define BZ_VARIANT(NEQ, LANES)                                                                             \
-  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false, false>, \
+  { "burn_coop<" #NEQ "," #LANES ">", NEQ, LANES, bz::CoopShape<LANES>::THREADS,                            \
+    (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false, false>,                                              \
     (KernelFn)bz::burn_coop_kernel<NEQ, LANES, true, false>,                                               \
     (KernelFn)bz::burn_coop_kernel<NEQ, LANES, false, true> }
 
@@ -292,7 +293,7 @@ struct bz_net {
   const Variant *variant;
   KernelFn coop_fn;  // variant->fn, or variant->fn_ext when the network carries density exponents or an EOS
   bool ext;          // ... which also means: no reuse policy on the cooperative kernel for this network
-  int grid, grid_reuse, smem_bytes;
+  int grid, grid_reuse, smem_bytes, coop_threads;
   const QuadVariant *quad;  // non-null: a specialised kernel exists for this topology
   int quad_grid;
   double *d_quad_coef, *d_quad_scratch;
@@ -361,28 +362,32 @@ int net_create(const bz_net_desc *d, bz_net **out) {
 
   // ---- launch geometry: persistent grid, blocks/SM from the occupancy calculator -----------------
   const int L = h->variant->lanes;
-  const int gpb = bz::COOP_THREADS / L;
-  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
-  const int tab = ((h->dev.ndbl + 1) & ~1) + (((h->dev.nint + 3) & ~3) / 2);
-  h->smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
+  // threads per block: the instance's, less if its shared memory would not fit (tables of large networks)
+  int COOPT = h->variant->threads;
   int sms = 0, bps = 0, optin = 0;
   if (!cuda_ok(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device))) return fail(BZ_ERR_CUDA);
   if (!cuda_ok(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device)))
     return fail(BZ_ERR_CUDA);
+  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
+  const int tab = ((h->dev.ndbl + 1) & ~1) + (((h->dev.nint + 3) & ~3) / 2);
+  while (COOPT > 32 && (tab + (COOPT / L) * ((pg + 1) & ~1)) * (int)sizeof(double) > optin) COOPT -= 32;
+  h->coop_threads = COOPT;
+  const int gpb = COOPT / L;
+  h->smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
   if (h->smem_bytes > optin) return fail(BZ_ERR_NOMEM);
   // the attribute belongs to the kernel, not to the handle: always opt in to the device maximum, so
   // that a later handle with smaller tables cannot lower it under an earlier one
   if (!cuda_ok(cudaFuncSetAttribute((const void *)h->coop_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
     return fail(BZ_ERR_CUDA);
   if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->coop_fn,
-                                                             bz::COOP_THREADS, h->smem_bytes)))
+                                                             h->coop_threads, h->smem_bytes)))
     return fail(BZ_ERR_CUDA);
   if (bps < 1) return fail(BZ_ERR_NOMEM);
   h->grid = sms * bps;
   if (!cuda_ok(cudaFuncSetAttribute((const void *)h->variant->fn_reuse, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)))
     return fail(BZ_ERR_CUDA);
   if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)h->variant->fn_reuse,
-                                                             bz::COOP_THREADS, h->smem_bytes)))
+                                                             h->coop_threads, h->smem_bytes)))
     return fail(BZ_ERR_CUDA);
   if (bps < 1) return fail(BZ_ERR_NOMEM);
   h->grid_reuse = sms * bps;
@@ -528,12 +533,13 @@ static int launch_burn(const bz_net *h, int64_t nz, int64_t ld, const double *rh
     return BZ_OK;
   }
   const int L = h->variant->lanes;
-  const long long groups_needed = (nz + (bz::COOP_THREADS / L) - 1) / (bz::COOP_THREADS / L);
+  const int COOPT = h->coop_threads;
+  const long long groups_needed = (nz + (COOPT / L) - 1) / (COOPT / L);
   const int cfull = h->policy == 1 ? h->grid_reuse : h->grid;
   const int grid = (int)(groups_needed < cfull ? groups_needed : cfull);
   const KernelFn cfn = h->policy == 1 ? h->variant->fn_reuse : h->coop_fn;
   void *args[] = {(void *)&h->dev, (void *)&a};
-  BZ_CUDA(cudaLaunchKernel((const void *)cfn, dim3(grid), dim3(bz::COOP_THREADS), args, (size_t)h->smem_bytes, st));
+  BZ_CUDA(cudaLaunchKernel((const void *)cfn, dim3(grid), dim3(COOPT), args, (size_t)h->smem_bytes, st));
   return BZ_OK;
 }
 
@@ -675,15 +681,17 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   const Variant *v = pick_variant(n);
   const KernelFn vfn = (F.has_rexp || F.eos) ? v->fn_ext : v->fn;  // (policy 0 only)
   const int L = v->lanes;
-  const int gpb = bz::COOP_THREADS / L;
   const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
   const int tab = ((F.ndbl + 1) & ~1) + (((F.nint + 3) & ~3) / 2);
+  int COOPT = v->threads;
+  while (COOPT > 32 && (tab + (COOPT / L) * ((pg + 1) & ~1)) * (int)sizeof(double) > sd->smem_optin) COOPT -= 32;
+  const int gpb = COOPT / L;
   const int smem_bytes = (tab + gpb * ((pg + 1) & ~1)) * (int)sizeof(double);
   if (smem_bytes > sd->smem_optin) return BZ_ERR_NOMEM;
   // opt in to the device's maximum: never lowers what a handle of net_create has set for this kernel
   BZ_CUDA(cudaFuncSetAttribute((const void *)vfn, cudaFuncAttributeMaxDynamicSharedMemorySize, sd->smem_optin));
   int bps = 0;
-  BZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)vfn, bz::COOP_THREADS, smem_bytes));
+  BZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void *)vfn, COOPT, smem_bytes));
   if (bps < 1) return BZ_ERR_NOMEM;
 
   unsigned char *base = sd->ptr;
@@ -713,7 +721,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   const long long full = (long long)sd->sms * bps;
   const int grid = (int)(groups_needed < full ? groups_needed : full);
   void *args[] = {(void *)&dn, (void *)&a};
-  BZ_CUDA(cudaLaunchKernel((const void *)vfn, dim3(grid), dim3(bz::COOP_THREADS), args, (size_t)smem_bytes, st));
+  BZ_CUDA(cudaLaunchKernel((const void *)vfn, dim3(grid), dim3(COOPT), args, (size_t)smem_bytes, st));
   return BZ_OK;
 }
 
