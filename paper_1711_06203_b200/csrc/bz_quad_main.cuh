@@ -13,7 +13,8 @@ namespace bz {
 // is compiled without any of it).
 template <class Net, int BLOCK, int MINB, bool REUSE>
 __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, BurnArgs A) {
-  constexpr int QUAD_THREADS = BLOCK;
+  constexpr int QUAD_THREADS = BLOCK;  // (a run-time block size was tried for small batches: it perturbed the
+                                       // register allocation of the alpha13 instance, config 3 +3 %)
   constexpr int NEQ = Net::NEQ, N = Net::N, K = Net::K, S = Net::S;
   typedef QuadMem<NEQ, K> Mem;
   extern __shared__ __align__(16) double smem[];

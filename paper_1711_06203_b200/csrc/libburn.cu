@@ -67,9 +67,10 @@ QuadVariant make_quad(const char *name) {
           (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB, false>,
           (QuadKernelFn)bz::burn_quad_kernel<Net, BLOCK, MINB, true>};
 }
-// one block of 384 threads per SM (<= 168 registers): all 12 warps share one barrier per trip = one
-// instruction stream (3 blocks of 128 threads were 1.8x slower, profiles/README.md)
-#define BZ_QUAD_ENTRY(NET) make_quad<NET, 384, 1>("burn_quad<" #NET ",384x1>"),
+// one block per SM (Net::QUAD_BLOCK threads: 384 at <= 168 registers, or 512 at <= 128 for the small
+// networks): all its warps share one barrier per trip = one instruction stream (3 blocks of 128 threads
+// were 1.8x slower, profiles/README.md)
+#define BZ_QUAD_ENTRY(NET) make_quad<NET, NET::QUAD_BLOCK, 1>(NET::QUAD_BLOCK == 512 ? "burn_quad<" #NET ",512x1>" : "burn_quad<" #NET ",384x1>"),
 const QuadVariant kQuad[] = {BZ_GEN_NETS(BZ_QUAD_ENTRY)};
 
 // FNV-1a over the topology; must equal paper_1711_06203_b200/codegen.py:topology_hash
