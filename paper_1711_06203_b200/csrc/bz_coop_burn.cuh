@@ -154,8 +154,26 @@ struct LuSmem {
       if (pos > k && lig < NEQ) {
         const double l = my * inv;
         row[k] = l;
-#pragma unroll 4
-        for (int j = k + 1; j < NEQ; j++) row[j] = fma_(-l, prow[j], row[j]);
+        // Loads staged by hand, four columns at a time, then two: written as row[j] = fma(-l, prow[j], row[j])
+        // the compiler must assume that row and prow overlap and chains load -> FMA -> store -> load, ~45
+        // cycles per column.  An odd number of columns takes the next one along -- index NEQ, padding of the
+        // row (NEQ < LD), updated and never read -- so that no column is left for a serial tail.
+        static_assert(NEQ < LD, "padding column");
+        int j = k + 1;
+        const int end = j + ((NEQ - j + 1) & ~1);
+#pragma unroll 1
+        for (; j + 4 <= end; j += 4) {
+          double p[4], r[4];
+#pragma unroll
+          for (int u = 0; u < 4; u++) p[u] = prow[j + u], r[u] = row[j + u];
+#pragma unroll
+          for (int u = 0; u < 4; u++) row[j + u] = fma_(-l, p[u], r[u]);
+        }
+        if (j < end) {
+          const double p0 = prow[j], p1 = prow[j + 1], r0 = row[j], r1 = row[j + 1];
+          row[j] = fma_(-l, p0, r0);
+          row[j + 1] = fma_(-l, p1, r1);
+        }
       }
     }
     g.sync();

@@ -169,7 +169,14 @@ __global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::M
         }
       }
     }
-    if (__syncthreads_and(phase == 2)) break;
+    // Sub-warp instances: one block barrier per trip (instruction cache, see the head of this file).  The
+    // warp-per-zone instances run free of each other: with the rolled in-place LU the hot part of a trip is
+    // ~70 KB of code and lockstep costs more than it saves (config 5 sample: 3 258 -> 2 883 ms; instruction-fetch
+    // stalls 10 % of the samples), and a warp leaves when the queue is empty (phase is warp-uniform there, and
+    // nothing else in the loop is block-wide).
+    if (LANES == 32) {
+      if (phase == 2) break;
+    } else if (__syncthreads_and(phase == 2)) break;
     if (phase == 1) {
 #include "bz_coop_attempt.inc"
     }
