@@ -117,11 +117,20 @@ __device__ __forceinline__ void select_eta(bool order_due, double etaq, double e
   }
 }
 
+// Row stride of a group's matrix M, in doubles: LANES + 1 (odd), so that the lanes of a group read one column,
+// or walk their own rows in step, without bank conflicts beyond the two wavefronts of a 64-bit access.
+// (Measured on config 5 and dropped: stride 34 with the rows walked by 128-bit accesses -- 3 instead of 6
+// instructions per FMA of the LU update, same bits, 2 904 ms instead of 2 787 ms: what is read by columns,
+// the pivot searches and the solves, then takes twice the wavefronts.)
+__host__ __device__ constexpr int coop_ld(int lanes) { return lanes + 1; }
+// per-group scratch, in doubles: M (LANES rows), urow (2 LANES), ysh, xs (LANES each), R, dRdT (K each), dRdY
+// (3 K); M on a 16-byte boundary wherever it is placed (burn_coop_kernel places it)
+__host__ __device__ constexpr int coop_per_group(int lanes, int K) { return lanes * coop_ld(lanes) + ((4 * lanes + 5 * K + 1) & ~1); }
+
 template <int NEQ, int LANES>
 struct CoopSmem {
-  // per-group scratch, in doubles
-  static constexpr int LD = LANES + 1;
-  __host__ __device__ static constexpr int per_group(int K) { return LANES /*ysh*/ + 5 * K /*R,dRdT,dRdY*/ + LANES * LD /*M*/ + 2 * LANES /*urow*/ + LANES /*xs*/; }
+  static constexpr int LD = coop_ld(LANES);
+  __host__ __device__ static constexpr int per_group(int K) { return coop_per_group(LANES, K); }
 };
 
 }  // namespace bz

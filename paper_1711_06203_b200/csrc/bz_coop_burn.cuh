@@ -19,7 +19,7 @@ struct LuRow {
   __device__ __forceinline__ void form(const G &g, double gamma, bool act, int n) {
 #pragma unroll
     for (int j = 0; j < NEQ; j++) {
-      const double Jij = (act && j < n) ? g.M[g.lig * (LANES + 1) + j] : 0.0;
+      const double Jij = (act && j < n) ? g.M[g.lig * CoopSmem<NEQ, LANES>::LD + j] : 0.0;
       a[j] = fma_(-gamma, Jij, (j == g.lig) ? 1.0 : 0.0);
     }
   }
@@ -103,7 +103,7 @@ struct LuRow {
 // broadcast buffer (urow) as ints.
 template <int NEQ, int LANES>
 struct LuSmem {
-  static constexpr int LD = LANES + 1;
+  static constexpr int LD = CoopSmem<NEQ, LANES>::LD;
   double myinv;  // 1/pivot of the step at which my row was the pivot row
   int pos;       // LINPACK position of my row
 

@@ -9,7 +9,7 @@ namespace bz {
 // them run the kernel without a trace of either (they cost 3.4 % of config 5 when compiled in).
 template <int NEQ, int LANES, bool EXT = false>
 struct Group {
-  static constexpr int LD = LANES + 1;
+  static constexpr int LD = CoopSmem<NEQ, LANES>::LD;
   // identity of this lane
   unsigned gmask;  // lanes of my group within the warp
   int lig;         // lane in group = component index

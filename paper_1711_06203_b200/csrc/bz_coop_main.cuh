@@ -31,7 +31,7 @@ struct CoopShape {
 template <int NEQ, int LANES, bool EXT, bool REUSE>
 __global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::MINB) burn_coop_kernel(DevNet net, BurnArgs A) {
   extern __shared__ __align__(16) double smem[];
-  constexpr int LD = LANES + 1;
+  constexpr int LD = CoopSmem<NEQ, LANES>::LD;
   const int N = net.N, n = net.n, K = net.K;
 
   // ---- block prologue: network tables -> shared memory ---------------------------------------
@@ -58,13 +58,18 @@ __global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::M
     const int pg = CoopSmem<NEQ, LANES>::per_group(K);
     const int pga = (pg + 1) & ~1;
     double *base = smem + tab + (threadIdx.x / LANES) * pga;
-    g.urow = base;                 // 2*LANES, 16-byte aligned
+    // M first for the sub-warp instances, last for the warp-per-zone ones: measured, the same kernel apart from
+    // address arithmetic (burn_coop<14,16> on config 3: 765 ms with M last, 741 ms with M first;
+    // burn_coop<31,32> on config 5: 2 777 ms with M last, 2 945 ms with M first)
+    constexpr int MSIZE = LANES * LD;  // even
+    const int rest = (4 * LANES + 5 * K + 1) & ~1;
+    g.M = (LANES == 32) ? base + rest : base;
+    g.urow = (LANES == 32) ? base : base + MSIZE;  // 2*LANES, 16-byte aligned
     g.ysh = g.urow + 2 * LANES;
     g.xs = g.ysh + LANES;
     g.R = g.xs + LANES;
     g.dRdT = g.R + K;
     g.dRdY = g.dRdT + K;
-    g.M = g.dRdY + 3 * K;
   }
   g.has_src = (A.src_T != nullptr);
   g.src = 0.0;

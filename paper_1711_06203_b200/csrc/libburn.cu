@@ -369,7 +369,7 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   if (!cuda_ok(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device))) return fail(BZ_ERR_CUDA);
   if (!cuda_ok(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device)))
     return fail(BZ_ERR_CUDA);
-  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
+  const int pg = bz::coop_per_group(L, K);
   const int tab = ((h->dev.ndbl + 1) & ~1) + (((h->dev.nint + 3) & ~3) / 2);
   while (COOPT > 32 && (tab + (COOPT / L) * ((pg + 1) & ~1)) * (int)sizeof(double) > optin) COOPT -= 32;
   h->coop_threads = COOPT;
@@ -682,7 +682,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   const Variant *v = pick_variant(n);
   const KernelFn vfn = (F.has_rexp || F.eos) ? v->fn_ext : v->fn;  // (policy 0 only)
   const int L = v->lanes;
-  const int pg = L + 5 * K + L * (L + 1) + 2 * L + L;
+  const int pg = bz::coop_per_group(L, K);
   const int tab = ((F.ndbl + 1) & ~1) + (((F.nint + 3) & ~3) / 2);
   int COOPT = v->threads;
   while (COOPT > 32 && (tab + (COOPT / L) * ((pg + 1) & ~1)) * (int)sizeof(double) > sd->smem_optin) COOPT -= 32;
