@@ -1,8 +1,8 @@
 // bz_coop_main.cuh -- kernel entry: persistent blocks, work queue, BZ-BDF v1 driver as a flat
-// state machine: one loop trip = one step attempt of the group's zone, and ONE block barrier per
-// trip keeps all warps of the block in the same part of the (large, unrolled) loop body so that
-// they share instruction-cache lines (profiles/README.md: unsynchronised warps stalled 8 cycles
-// per issue on instruction fetch).
+// state machine: one loop trip = one step attempt of the group's zone.  In the sub-warp instances ONE
+// block barrier per trip keeps all warps of the block in the same part of the (large, unrolled) loop
+// body so that they share instruction-cache lines (profiles/README.md: unsynchronised warps stalled 8
+// cycles per issue on instruction fetch); the warp-per-zone instances, whose LU is rolled, run without.
 #pragma once
 #include "bz_coop_burn.cuh"
 
@@ -20,11 +20,10 @@ struct CoopShape {
   static constexpr int THREADS = (LANES == 32) ? 512 : COOP_THREADS;
   static constexpr int MINB = (LANES == 32) ? 1 : 2;
 };
-// Blocks per SM: the warp-per-zone instances (LANES == 32: a row of up to 32 doubles per lane) need the
-// full 255 registers, one block per SM; with 128 registers they spill 1.7 KB per thread and ran 28 %
-// slower.  The sub-warp instances fit 128 registers, and two blocks per SM (16 warps instead of 8) ran
-// 9 % faster (config 3 on burn_coop<14,16>) -- when shared memory allows two blocks, which net_create
-// asks the occupancy calculator.
+// Blocks per SM: the warp-per-zone instances take one block of 16 warps (registers and shared memory both
+// full).  The sub-warp instances fit 128 registers, and two blocks per SM (16 warps instead of 8) ran 9 %
+// faster (config 3 on burn_coop<14,16>) -- when shared memory allows two blocks, which net_create asks the
+// occupancy calculator.
 // REUSE: the Newton-matrix policy of bz_set_policy(net, 1), a separate instantiation.  A
 // group owns its zone's factors (LuRow, registers) and nothing of them is shared across groups, so a
 // group that keeps its matrix simply skips Jacobian and LU: no warp-level sharing as in the quad kernel.
