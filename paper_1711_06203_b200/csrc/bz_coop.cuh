@@ -1,15 +1,15 @@
 // bz_coop.cuh -- cooperative burn kernel: LANES threads of a warp integrate one zone.
 //
 // Mapping: lane i of a group owns component i of every n-vector
-// (Nordsieck rows, weights, corrections) and ROW i of the Newton matrix P = I - gamma*J, all in
-// registers.  A warp holds 32/LANES zones.  Groups pull zones from a global atomic work queue
+// (Nordsieck rows, weights, corrections) in registers and ROW i of the Newton matrix P = I - gamma*J
+// in the group's shared-memory matrix.  A warp holds 32/LANES zones.  Groups pull zones from a global atomic work queue
 // (step a2: compaction against step-count divergence -- a group that finishes its zone fetches
 // the next one, so co-resident zones never wait for the slowest of a fixed batch).
 //   a3/a4 rates + Jacobian: reactions are dealt round-robin to lanes (one exp each), the
 //         per-reaction rate and partials go through shared memory, then lane i gathers row i.
-//   a5    LU: implicit row pivoting (rows never move; each lane carries its LINPACK position
-//         `pos`), pivot search by a 64-bit max butterfly, pivot row broadcast through shared
-//         memory, rank-1 update of the lane's own row with fma.
+//   a5    LU: in place in shared memory, implicit row pivoting (rows never move; each lane carries its
+//         LINPACK position `pos`), pivot search by a 64-bit maximum over the group, the pivot row read
+//         where it lies, rank-1 update of the lane's own row with fma.
 //   a6    solves: dgesl order; the pivot component is broadcast by shuffle.
 //   a7/a8 BDF bookkeeping: per lane on its own component; step/order control is computed
 //         redundantly by every lane of the group (identical bits, no communication).

@@ -4,103 +4,19 @@
 
 namespace bz {
 
-// Per-lane view of the factorised Newton matrix.
-template <int NEQ, int LANES>
-struct LuRow {
-  double a[NEQ];  // my row: multipliers l_ik (k < pos), then U (k >= pos)
-  double myinv;   // 1/pivot of the step at which my row was the pivot row
-  int pos;        // LINPACK position of my row (= step at which it became the pivot row)
-  unsigned plpack[(NEQ + 3) / 4];  // pivot lane of every step, 8 bits each
-
-  __device__ __forceinline__ int pivot_lane(int k) const { return (plpack[k >> 2] >> ((k & 3) * 8)) & 0xff; }
-
-  // my row of P = I - gamma*J, from the row of J that the rates left in the group's matrix M
-  template <class G>
-  __device__ __forceinline__ void form(const G &g, double gamma, bool act, int n) {
-#pragma unroll
-    for (int j = 0; j < NEQ; j++) {
-      const double Jij = (act && j < n) ? g.M[g.lig * CoopSmem<NEQ, LANES>::LD + j] : 0.0;
-      a[j] = fma_(-gamma, Jij, (j == g.lig) ? 1.0 : 0.0);
-    }
-  }
-
-  // a5: in-place LU with partial pivoting, LINPACK tie-break (first maximal |a_ik| in the
-  // current row order), rows never move.  Returns false if a pivot column is all zero.
-  template <class G>
-  __device__ __forceinline__ bool factor(const G &g) {
-    const int lig = g.lig;
-    pos = lig;
-    myinv = 0.0;
-    bool ok = true;
-#pragma unroll
-    for (int w = 0; w < (NEQ + 3) / 4; w++) plpack[w] = 0u;
-#pragma unroll
-    for (int k = 0; k < NEQ; k++) {
-      const bool cand0 = (pos >= k) && (lig < NEQ);
-      const unsigned long long key =
-          cand0 ? (unsigned long long)(__double_as_longlong(a[k]) & 0x7fffffffffffffffLL) : 0ull;
-      const unsigned long long kmax = g.gmax(key);
-      if (kmax == 0ull || kmax > 0x7ff0000000000000ull) ok = false;  // zero or NaN pivot column
-      const bool cand = cand0 && (key == kmax);
-      unsigned ball = g.gballot(cand);
-      if (__popc(ball) > 1) {  // exact tie: smallest LINPACK position wins
-        const int mp = g.gmin(cand ? pos : 0x7fffffff);
-        ball = g.gballot(cand && pos == mp);
-      }
-      const int pl = __ffs(ball) - 1;
-      plpack[k >> 2] |= (unsigned)(pl & 0xff) << ((k & 3) * 8);
-      const int ppos = __shfl_sync(g.gmask, pos, pl & (LANES - 1), LANES);
-      const bool isp = (lig == pl);
-      if (pos == k) pos = ppos;
-      if (isp) pos = k;
-      double *ub = g.urow + (k & 1) * LANES;
-      if (isp) {
-#pragma unroll
-        for (int j = k; j < NEQ; j++) ub[j] = a[j];
-      }
-      g.sync();
-      const double inv = 1.0 / ub[k];
-      if (isp) myinv = inv;
-      if (pos > k) {
-        const double l = a[k] * inv;
-        a[k] = l;
-#pragma unroll
-        for (int j = k + 1; j < NEQ; j++) a[j] = fma_(-l, ub[j], a[j]);
-      }
-    }
-    return ok;
-  }
-
-  // a6: solve P x = b (dgesl order).  b = my component on entry, x_lig on return.
-  template <class G>
-  __device__ __forceinline__ double solve(const G &g, double b) const {
-#pragma unroll
-    for (int k = 0; k < NEQ; k++) {
-      const double bk = g.bcast(b, pivot_lane(k));
-      if (pos > k) b = fma_(-a[k], bk, b);
-    }
-#pragma unroll
-    for (int k = NEQ - 1; k >= 0; k--) {
-      const double x = b * myinv;
-      if (pos == k) b = x;
-      const double xk = g.bcast(x, pivot_lane(k));
-      if (pos < k) b = fma_(-a[k], xk, b);
-    }
-    // x_j sits on the lane whose row has position j: route it to lane j
-    g.sync();
-    if (g.lig < NEQ) g.xs[pos] = b;
-    g.sync();
-    return (g.lig < NEQ) ? g.xs[g.lig] : 0.0;
-  }
-};
-
-// The same factorisation with the rows left where the rates put them: in the group's shared-memory
-// matrix M (lane i owns row i at M + i*LD, LD = LANES + 1: lanes i and i + 16 share a bank, the minimum
-// for 64-bit accesses).  A warp-per-zone lane then carries no row in registers (62 of them for n = 31),
-// the pivot row is read where it lies instead of being published to a broadcast buffer, and the loops
-// over k and j are rolled: the factorisation is 2 KB of code instead of 54 KB.  Operations and their
-// order are those of LuRow: same bits.  The pivot lanes of the steps are kept in the group's old
-// broadcast buffer (urow) as ints.
+// The factorised Newton matrix of a group's zone, in place in the group's shared-memory matrix M, where the
+// rates left the rows of J: lane i owns row i at M + i*LD (LD = LANES + 1: the lanes of a group walk their rows
+// in step, or read one column, without bank conflicts beyond the two wavefronts of a 64-bit access).
+// a5: LU with partial pivoting, LINPACK tie-break (first maximal |a_ik| in the current row order); rows never
+// move: each lane carries the LINPACK position of its row (= the step at which it became the pivot row) and
+// the pivot lanes of the steps are kept as ints in the group's buffer urow; the pivot row is read where it
+// lies.  The loops over k and j are rolled: 2 KB of code.
+// Round 1 and most of round 2 kept each lane's row in REGISTERS instead (static indices, everything unrolled:
+// 54 KB of code for n = 31, 62 registers for the row, the pivot row published through a double-buffered
+// broadcast buffer).  Same operations in the same order, same bits, and slower on every instance, because the
+// row's registers and the size of the code cost more than the shared-memory traffic of this form:
+// burn_coop<31,32> 3 447 -> 3 258 ms (twice the warps at 128 registers), <14,16> 747 -> 555 ms, <8,8> 471 -> 387
+// ms, <3,4> 415 -> 372 ms (configs 5, 3, 2 and 1's networks on the generic kernel).
 template <int NEQ, int LANES>
 struct LuSmem {
   static constexpr int LD = CoopSmem<NEQ, LANES>::LD;
@@ -201,15 +117,6 @@ struct LuSmem {
     g.sync();
     return (g.lig < NEQ) ? g.xs[g.lig] : 0.0;
   }
-};
-
-template <int NEQ, int LANES, bool SMEM = (LANES == 32)>
-struct LuPick {
-  typedef LuRow<NEQ, LANES> type;
-};
-template <int NEQ, int LANES>
-struct LuPick<NEQ, LANES, true> {
-  typedef LuSmem<NEQ, LANES> type;
 };
 
 // Nordsieck helpers on my component.  Arrays are indexed with compile-time indices only.

@@ -1,20 +1,21 @@
 // bz_coop_main.cuh -- kernel entry: persistent blocks, work queue, BZ-BDF v1 driver as a flat
 // state machine: one loop trip = one step attempt of the group's zone.  In the sub-warp instances ONE
-// block barrier per trip keeps all warps of the block in the same part of the (large, unrolled) loop
-// body so that they share instruction-cache lines (profiles/README.md: unsynchronised warps stalled 8
-// cycles per issue on instruction fetch); the warp-per-zone instances, whose LU is rolled, run without.
+// block barrier per trip keeps all warps of the block in the same part of the (large) loop body so that
+// they share instruction-cache lines (profiles/README.md: unsynchronised warps stalled 8 cycles per issue
+// on instruction fetch; still 713 against 555 ms for burn_coop<14,16> with the rolled LU); the
+// warp-per-zone instances run without (see the loop).
 #pragma once
 #include "bz_coop_burn.cuh"
 
 namespace bz {
 
 constexpr int COOP_THREADS = 256;
-// Threads per block of an instance.  The warp-per-zone instances factorise in place in the group's
-// shared-memory matrix (LuSmem, bz_coop_burn.cuh), which takes the 31-entry row out of every lane's
-// registers: 128 registers instead of 255, so one block holds 16 zones (16 warps) instead of 8.  Measured on
-// config 5 (131 072-zone sample): rows in registers, 256 threads 3 447 ms; rows in shared memory, 256
-// threads 4 290 ms (two loads and a store per FMA), 384 threads 3 415 ms, 512 threads 3 258 ms.  net_create
-// launches fewer threads when the tables of a large network leave no room for 16 groups.
+// Threads per block of an instance.  The LU lives in the group's shared-memory matrix (LuSmem,
+// bz_coop_burn.cuh), so a warp-per-zone lane carries no 31-entry row: 128 registers instead of 255, and one
+// block holds 16 zones (16 warps) instead of 8.  Measured on config 5 (131 072-zone sample): rows in
+// registers, 256 threads 3 447 ms; rows in shared memory, 256 threads 4 290 ms, 384 threads 3 415 ms, 512
+// threads 3 258 ms.  net_create launches fewer threads when the tables of a large network leave no room for
+// 16 groups.
 template <int LANES>
 struct CoopShape {
   static constexpr int THREADS = (LANES == 32) ? 512 : COOP_THREADS;
@@ -25,8 +26,9 @@ struct CoopShape {
 // faster (config 3 on burn_coop<14,16>) -- when shared memory allows two blocks, which net_create asks the
 // occupancy calculator.
 // REUSE: the Newton-matrix policy of bz_set_policy(net, 1), a separate instantiation.  A
-// group owns its zone's factors (LuRow, registers) and nothing of them is shared across groups, so a
-// group that keeps its matrix simply skips Jacobian and LU: no warp-level sharing as in the quad kernel.
+// group owns its zone's factors (in its matrix M, which only a fresh Jacobian overwrites) and nothing of them
+// is shared across groups, so a group that keeps its matrix simply skips Jacobian and LU: no warp-level
+// sharing as in the quad kernel.
 template <int NEQ, int LANES, bool EXT, bool REUSE>
 __global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::MINB) burn_coop_kernel(DevNet net, BurnArgs A) {
   extern __shared__ __align__(16) double smem[];
@@ -77,8 +79,7 @@ __global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::M
   const double dt = A.dt, rtol = A.rtol, atol = A.atol;
   unsigned long long c_nst = 0, c_rhs = 0, c_jac = 0, c_lu = 0, c_sol = 0, c_etf = 0, c_cfn = 0, c_fail = 0;
 
-  // warp-per-zone instances factorise in place in shared memory, sub-warp instances in registers
-  typename LuPick<NEQ, LANES>::type lu;
+  LuSmem<NEQ, LANES> lu;  // the factors live in g.M; the lane keeps its row's position and 1/pivot
 
   // per-zone integrator state, persistent across loop trips (registers; uniform within the group
   // except the per-component Z, w, S)
