@@ -2,7 +2,7 @@
 """bench.py -- zones burned/sec on the 13-isotope 128^3 config (BASELINE.json configs[2]).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
-                    [--static-schedule] [--kernel auto|coop|quad]
+                    [--static-schedule] [--kernel auto|coop|quad] [--order cost|index|steps]
 
 A "step" is one pass of the whole hot path (a1-a9: load, work queue, rates, Jacobian, LU,
 Newton, BDF control, store) over one batch of synthetic zones: one burn_zones call.
@@ -167,9 +167,14 @@ def run_ours(args):
     nz, N = w.nz, w.net.nspec
     net = bz.net_create(w.net)
     net.select_kernel(args.kernel)
-    net.set_schedule("static" if args.static_schedule else "queue")
+    net.set_schedule("static" if args.static_schedule else ("cost" if args.order == "cost" else "queue"))
     net.set_policy(args.policy)
     stream = torch.cuda.current_stream()
+    order_note = "zone index (bz_set_schedule 0)"
+    if args.order == "cost" and not args.static_schedule:
+        # the library's default: its own a-priori key, key kernel + radix sort INSIDE every timed burn
+        order_note = ("by decreasing a-priori cost key |dT/dt| / T at the initial state (bz_set_schedule 2, the default: "
+                      "one right-hand side per zone and a radix sort, inside the timed burn)")
 
     # ---- device-resident arm -------------------------------------------------------------------
     rho_d, T_d, X_d = (torch.from_numpy(a).to(dev) for a in (w.rho, w.T, w.X))
@@ -183,6 +188,15 @@ def run_ours(args):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.order == "steps":
+        # a caller's order (bz_set_zone_order): by decreasing step count of a PREVIOUS burn of this batch -- what an
+        # application that burns every hydro step knows from the step before; on a repeated identical batch it is
+        # the ideal key.  Results do not depend on it.
+        step()
+        torch.cuda.synchronize()
+        net.set_zone_order(torch.argsort(ns_d.to(torch.int64), descending=True, stable=True))
+        order_note = "by decreasing step count of a previous burn of the same batch (a caller's order; ideal cost key)"
 
     for _ in range(args.warmup):
         step()
@@ -203,6 +217,7 @@ def run_ours(args):
     nfail = int((ns_d < 0).sum().item())
 
     # ---- end-to-end arm: host buffers through the C ABI, copies inside the timed region --------
+    net.set_zone_order(None)   # (the host path burns in chunks and takes no caller's order)
     pin = lambda a: torch.from_numpy(a).pin_memory()
     rho_h, T_h, X_h = pin(w.rho), pin(w.T), pin(w.X)
     To_h = torch.empty(nz, dtype=torch.float64).pin_memory()
@@ -248,7 +263,7 @@ def run_ours(args):
         tpath = os.path.join(ROOT, "profiles", "ncu_counters.json")
         if os.path.exists(tpath):
             rec = json.load(open(tpath)).get(f"config{cfg}:{net.kernel_name}")
-            if rec and not args.static_schedule and args.policy == "fresh":
+            if rec and not args.static_schedule and args.policy == "fresh" and args.order == "cost":
                 traffic, executed, ncu_src = rec.get("dram_bytes"), rec.get("executed_fp64_flops"), rec.get("source")
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -258,6 +273,7 @@ def run_ours(args):
                        "zones_per_gpu": nz, "neq": N + 1, "nreac": w.net.nreac,
                        "dt": w.dt, "rtol": w.rtol, "atol": w.atol, "kernel": net.kernel_name,
                        "schedule": "static round-robin (a2 off)" if args.static_schedule else "work queue (a2)",
+                       "queue_order": order_note,
                        "newton_matrix": "fresh J + LU every attempt (BZ-BDF v1)" if args.policy == "fresh"
                                         else "reused, VODE-style (BZ-BDF v2, DESIGN.md 12)",
                        "l2": (f"inputs {8 * (N + 2) * nz / 1e6:.0f} MB per step exceed the 126 MB L2" if 8 * (N + 2) * nz > 126e6
@@ -281,7 +297,9 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms,
                     "h2d_bytes_per_step": 8 * (N + 2) * nz, "d2h_bytes_per_step": (8 * (N + 1) + 4) * nz,
                     "matches_device_path": same},
-            "gpu_launches": args.steps, "clocks": clocks,
+            # kernels of this repository inside the timed region: the burn kernel, and with the cost schedule the
+            # key kernel before it (the radix sort between them is CUB's: 3-4 library kernels per step, not counted)
+            "gpu_launches": args.steps * (2 if (args.order == "cost" and not args.static_schedule) else 1), "clocks": clocks,
         }
         if not args.no_cpu_baseline and world == 1:
             import oracle
@@ -331,6 +349,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", default="auto", choices=["auto", "coop", "quad"],
                     help="auto = specialised quad kernel when the topology has one, else the generic coop kernel")
+    ap.add_argument("--order", default="cost", choices=["cost", "index", "steps"],
+                    help="order in which the work queue hands the zones out: the library's a-priori cost key (default, "
+                         "bz_set_schedule 2), zone index (bz_set_schedule 0), or decreasing step count of a previous "
+                         "burn of the batch (bz_set_zone_order; device-resident arm only)")
     ap.add_argument("--static-schedule", action="store_true",
                     help="switch the work queue (step a2) off: static round-robin zone assignment, for the before/after figure")
     ap.add_argument("--policy", default="fresh", choices=["fresh", "reuse"],

@@ -175,11 +175,39 @@ int bz_norm_lanes(const bz_net *net);
 int bz_select_kernel(bz_net *net, int kind);
 
 /* Zone scheduling (step a2, "a lot of thread divergence due to the widely differing thermodynamic
- * conditions"): kind 0 (default) = a global work queue -- a lane group that finishes
- * its zone fetches the next one, so co-resident zones never wait for the slowest of a fixed batch;
- * kind 1 = static round-robin assignment (group g burns zones g, g + G, g + 2G, ...), kept only so
- * that the benefit of the queue can be MEASURED (bench.py --static-schedule).  Results are identical. */
+ * conditions").  A global work queue: a lane group that finishes its zone fetches the next
+ * one, so co-resident zones never wait for the slowest of a fixed batch.
+ *   kind 2 (default): the queue hands the zones out by decreasing a-priori COST KEY:
+ *          |sum_k Q_k R_k| / T at the initial state, the relative heating rate up to common factors, from one
+ *          right-hand side per zone in a kernel of its own, then one device radix sort of (key, index) pairs
+ *          on the key's upper 16 bits -- both inside the burn call, on its stream.  Dear zones start first
+ *          and zones of similar cost run side by side.  Config 4: 78.6 -> 46.2 ms per call; config 3: 1 958 ->
+ *          1 932 ms.  Needs 24 bytes per zone of device memory, owned by the handle, allocated at
+ *          the first call and when a batch is larger than any before (those calls synchronise the stream); if
+ *          that memory is not to be had, if nz >= 2^31, or if the grid takes all zones at once, the call
+ *          burns in index order.  burn_zones_static never orders (it allocates nothing).
+ *   kind 0: the queue hands the zones out in index order.
+ *   kind 1: static round-robin assignment (group g burns zones g, g + G, g + 2G, ...), kept only so that the
+ *          benefit of the queue can be MEASURED (bench.py --static-schedule).
+ * Every zone's result is bit-identical under all three; only the time differs. */
 int bz_set_schedule(bz_net *net, int kind);
+
+/* A caller's own ORDER for the work queue, instead of the library's cost key (e.g. the step counts of the
+ * previous hydro step's burn, which the library cannot know).  order: DEVICE pointer to nz int64 entries, a permutation of 0 .. nz-1 -- the q-th zone
+ * taken from the queue is zone order[q] -- or NULL (with nz = 0) to return to the handle's schedule.  The
+ * library keeps the pointer, not a copy: the array is the caller's and must stay valid and unchanged until
+ * the burns that use it have completed; it applies to every later burn_zones / burn_zones_src call of this
+ * handle, whose nz must equal the nz given here (else BZ_ERR_SIZE); burn_zones_host and the static schedule
+ * refuse it (BZ_ERR_UNSUPPORTED); burn_zones_static never uses it.  Zones are independent, so every zone's
+ * result is bit-identical whatever the order, and outputs stay at the zone's own index; only the time
+ * changes: zones that take a similar number of steps and start together stay in phase, and a warp's
+ * attempt then runs the rare paths (second Newton iteration, order change, rescale) for fewer of its zones
+ * at a time.  Config 3, order = zones by decreasing step count of a previous burn of the same batch:
+ * 1 958 -> 1 742 ms, against 1 932 ms with the library's a-priori key.
+ * The entries are not checked on the host; an entry outside [0, nz) is ignored by the kernel, and a zone that
+ * no entry names is not burned (its outputs are left untouched).
+ * Errors: BZ_ERR_NULL (net), BZ_ERR_SIZE (nz < 0, or order NULL with nz != 0). */
+int bz_set_zone_order(bz_net *net, const int64_t *order, int64_t nz);
 
 /* Newton-matrix policy ("we ported our workhorse ODE integrator (VODE [33])",
  * PAPER.md:L119, and VODE reuses its factorised Newton matrix, ref. [33] L184).

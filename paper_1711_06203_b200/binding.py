@@ -11,7 +11,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 COUNTER_NAMES = ("nst", "nrhs", "njac", "nlu", "nsolve", "netf", "ncfn", "nfailzones")
 EXPORTED_SYMBOLS = ("net_create", "burn_zones", "burn_zones_src", "burn_zones_host", "burn_zones_static", "net_destroy",
                     "bz_get_counters",
-                    "bz_norm_lanes", "bz_select_kernel", "bz_set_schedule", "bz_set_limits", "bz_set_policy", "bz_kernel_name",
+                    "bz_norm_lanes", "bz_select_kernel", "bz_set_schedule", "bz_set_zone_order", "bz_set_limits", "bz_set_policy",
+                    "bz_kernel_name",
                     "bz_last_cuda_error", "bz_fp64_peak_probe")
 _STATUS = {-1: "null pointer", -2: "bad size", -3: "bad network", -4: "bad scalar",
            -5: "CUDA runtime error", -6: "out of memory", -7: "unsupported", -8: "handle belongs to another device"}
@@ -76,6 +77,8 @@ def _L():
         lib.bz_select_kernel.argtypes = [vp, C.c_int]
         lib.bz_set_schedule.restype = C.c_int
         lib.bz_set_schedule.argtypes = [vp, C.c_int]
+        lib.bz_set_zone_order.restype = C.c_int
+        lib.bz_set_zone_order.argtypes = [vp, C.c_void_p, C.c_int64]
         lib.bz_set_policy.restype = C.c_int
         lib.bz_set_policy.argtypes = [vp, C.c_int]
         lib.bz_set_limits.restype = C.c_int
@@ -114,9 +117,35 @@ class Net:
         """'auto' (specialised quad kernel when available), 'coop' (generic), 'quad'."""
         _check(_L().bz_select_kernel(self._h, {"auto": 0, "coop": 1, "quad": 3}[kind]), "bz_select_kernel")
 
-    def set_schedule(self, kind: str = "queue") -> None:
-        """'queue' (work queue, default) or 'static' (round-robin assignment; for measuring a2)."""
-        _check(_L().bz_set_schedule(self._h, {"queue": 0, "static": 1}[kind]), "bz_set_schedule")
+    def set_schedule(self, kind: str = "cost") -> None:
+        """'cost' (work queue, zones handed out dearest first by the library's a-priori cost key; the default of
+        a new handle), 'queue' (work queue in index order) or 'static' (round-robin assignment; for measuring a2)."""
+        _check(_L().bz_set_schedule(self._h, {"queue": 0, "static": 1, "cost": 2}[kind]), "bz_set_schedule")
+
+    def set_zone_order(self, order=None, validate: bool = True) -> None:
+        """The order in which the work queue hands the zones out: a CUDA int64 tensor holding a permutation
+        of 0..nz-1 (e.g. ``torch.argsort(nsteps_of_the_previous_burn, descending=True)``), or None for
+        index order.  Applies to the later burn_zones / burn_zones_src calls of this handle on batches of
+        exactly that many zones.  Results do not depend on it, only the time does (include/burnzones.h).
+        The tensor is kept alive by the handle; do not modify it while burns that use it are in flight."""
+        if order is None:
+            _check(_L().bz_set_zone_order(self._h, None, 0), "bz_set_zone_order")
+            self._order = None
+            return
+        import torch
+        if not (isinstance(order, torch.Tensor) and order.is_cuda and order.dtype == torch.int64 and order.dim() == 1
+                and order.is_contiguous()):
+            raise ValueError("order: a contiguous 1-d CUDA int64 tensor")
+        nz = order.numel()
+        if validate and nz > 0:
+            seen = torch.zeros(nz, dtype=torch.bool, device=order.device)
+            if int(order.min()) < 0 or int(order.max()) >= nz:
+                raise ValueError("order: entries outside 0..nz-1")
+            seen[order] = True
+            if not bool(seen.all()):
+                raise ValueError("order: not a permutation of 0..nz-1")
+        _check(_L().bz_set_zone_order(self._h, order.data_ptr(), nz), "bz_set_zone_order")
+        self._order = order
 
     def set_policy(self, kind: str = "fresh") -> None:
         """'fresh' (Jacobian + LU on every attempt, default) or 'reuse' (VODE-style kept Newton matrix;

@@ -57,6 +57,7 @@ struct BurnArgs {
   const double *src_T, *src_X;   // constant source terms (burn_zones_src), both nullptr = none
   int mxstep, mxnef, mxncf;      // limits behind the failure codes -3 / -2 / -1 (bz_set_limits)
   int static_sched;              // 1: static round-robin zone assignment instead of the work queue (bz_set_schedule)
+  const long long *order;        // nullptr, or the order in which the queue hands the zones out (bz_set_zone_order)
 };
 
 __device__ __forceinline__ double inv_small_int(int p) {  // 1.0/p, p = 1..7, correctly rounded

@@ -109,12 +109,18 @@ __global__ void __launch_bounds__(CoopShape<LANES>::THREADS, CoopShape<LANES>::M
         z = started ? z + G : (long long)blockIdx.x * (blockDim.x / LANES) + threadIdx.x / LANES;
         started = true;
       } else {
-        if (lig == 0) z = (long long)atomicAdd(A.queue, 1ull);
+        if (lig == 0) {
+          z = (long long)atomicAdd(A.queue, 1ull);
+          if (A.order != nullptr && z < A.nz) {  // bz_set_zone_order: the q-th zone handed out is order[q]
+            z = A.order[z];
+            if ((unsigned long long)z >= (unsigned long long)A.nz) z = -1;  // not a zone: ignored
+          }
+        }
         z = __shfl_sync(g.gmask, z, 0, LANES);
       }
       if (z >= A.nz) {
         phase = 2;
-      } else {
+      } else if (z >= 0) {
         // ---- a1: load zone state -----------------------------------------------------------------
         rho = A.rho[z];
         double xin = 0.0;

@@ -105,13 +105,18 @@ __global__ void __launch_bounds__(BLOCK, MINB) burn_quad_kernel(QuadNet qn, Burn
       // (bz_set_schedule(1) switches the queue off for the before/after measurement of a2: quad g then
       // burns zones g, g + G, g + 2G, ... with G = quads of the grid; same results, different balance)
       long long z = 0;
-      if (c == 0)
+      if (c == 0) {
         z = A.static_sched ? m.zid() + (long long)gridDim.x * (QUAD_THREADS / 4) : (long long)atomicAdd(A.queue, 1ull);
+        if (A.order != nullptr && z < A.nz) {  // bz_set_zone_order: the q-th zone handed out is order[q]
+          z = A.order[z];
+          if ((unsigned long long)z >= (unsigned long long)A.nz) z = -1;  // not a zone: ignored
+        }
+      }
       z = __shfl_sync(gmask, z, 0, 4);
       m.zid() = z;
       if (z >= A.nz) {
         phase = 2;
-      } else {
+      } else if (z >= 0) {
         rho = A.rho[z];
         double xin[S], y[S];
         bool bad = !(rho > 0.0) || !finite_(rho);

@@ -9,10 +9,12 @@
 #include <vector>
 
 #include <cuda_runtime.h>
+#include <cub/device/device_radix_sort.cuh>
 
 #include "../../include/burnzones.h"
 #include "bz_coop_main.cuh"
 #include "bz_quad_main.cuh"
+#include "bz_cost_key.cuh"
 #include "gen/registry.inc"
 
 namespace {
@@ -301,7 +303,16 @@ struct bz_net {
   double fac;
   int kind;        // 0 auto, 1 cooperative, 3 quad (bz_select_kernel)
   int device;      // the device that was current at net_create: a handle belongs to ONE device
-  int static_sched;  // bz_set_schedule: 0 = work queue (a2), 1 = static round-robin assignment
+  int static_sched;  // bz_set_schedule: 0 = work queue in index order, 1 = static round-robin, 2 = work queue in cost order
+  const long long *order;  // bz_set_zone_order: device array (caller's), or nullptr
+  long long order_nz;
+  // bz_set_schedule 2: buffers of the library's own cost order, grown on demand (mutable: the burn entry points
+  // take a const handle, and a handle serves one burn at a time as its queue and counters already require)
+  mutable unsigned *ck_key[2];
+  mutable long long *ck_idx[2];
+  mutable void *ck_tmp;
+  mutable size_t ck_tmp_bytes;
+  mutable long long ck_cap;
   int mxstep, mxnef, mxncf;  // bz_set_limits
   int policy;                // bz_set_policy: 0 fresh matrix every attempt, 1 reuse
   int quad_grid_reuse;
@@ -333,6 +344,7 @@ int net_create(const bz_net_desc *d, bz_net **out) {
   bz_net *h = new (std::nothrow) bz_net();
   if (!h) return BZ_ERR_NOMEM;
   std::memset(h, 0, sizeof(*h));
+  h->static_sched = 2;  // the work queue, zones handed out in the library's cost order (bz_set_schedule)
   h->N = N; h->n = n; h->K = K;
   h->variant = pick_variant(n);
   h->ext = (F.has_rexp || F.eos);
@@ -440,6 +452,11 @@ int net_destroy(bz_net *h) {
   if (h->d_scratch) cudaFree(h->d_scratch);
   if (h->d_quad_coef) cudaFree(h->d_quad_coef);
   if (h->d_quad_scratch) cudaFree(h->d_quad_scratch);
+  for (int i = 0; i < 2; i++) {
+    if (h->ck_key[i]) cudaFree(h->ck_key[i]);
+    if (h->ck_idx[i]) cudaFree(h->ck_idx[i]);
+  }
+  if (h->ck_tmp) cudaFree(h->ck_tmp);
   if (h->st_in) cudaFree(h->st_in);
   if (h->st_out) cudaFree(h->st_out);
   if (h->st_nsteps) cudaFree(h->st_nsteps);
@@ -468,8 +485,15 @@ int bz_select_kernel(bz_net *h, int kind) {
 }
 int bz_set_schedule(bz_net *h, int kind) {
   if (!h) return BZ_ERR_NULL;
-  if (kind != 0 && kind != 1) return BZ_ERR_SIZE;
+  if (kind != 0 && kind != 1 && kind != 2) return BZ_ERR_SIZE;
   h->static_sched = kind;
+  return BZ_OK;
+}
+int bz_set_zone_order(bz_net *h, const int64_t *order, int64_t nz) {
+  if (!h) return BZ_ERR_NULL;
+  if (nz < 0 || (order == nullptr && nz != 0)) return BZ_ERR_SIZE;
+  h->order = reinterpret_cast<const long long *>(order);
+  h->order_nz = order ? nz : 0;
   return BZ_OK;
 }
 int bz_set_policy(bz_net *h, int kind) {
@@ -505,6 +529,50 @@ static bool scalars_ok(double dt, double rtol, double atol) {
   return (dt > 0.0) && (rtol > 0.0) && (atol >= 0.0) && std::isfinite(dt) && std::isfinite(rtol) && std::isfinite(atol);
 }
 
+// bz_set_schedule 2: the zones of this launch by decreasing cost key (bz_cost_key.cuh), in *order.  A key kernel
+// and one radix sort of (key, index) pairs on the key's upper 16 bits (11 exponent + 4 mantissa bits: zones
+// within 6 % of each other's key keep their index order; the sort is stable and deterministic).
+static int cost_order(const bz_net *h, int64_t nz, int64_t ld, const double *rho, const double *T, const double *X,
+                      cudaStream_t st, const long long **order) {
+  *order = nullptr;  // index order: what every soft failure below falls back to (the order is an aid, not a result)
+  if (nz > 0x7fffffffLL) return BZ_OK;
+  size_t need = 0;
+  BZ_CUDA(cub::DeviceRadixSort::SortPairsDescending(nullptr, need, (const unsigned *)nullptr, (unsigned *)nullptr,
+                                                    (const long long *)nullptr, (long long *)nullptr, (int)nz, 16, 32, st));
+  if (h->ck_cap < nz || h->ck_tmp_bytes < need) {
+    BZ_CUDA(cudaStreamSynchronize(st));  // nothing of an earlier burn on this stream still reads the old buffers
+    auto drop = [&]() {
+      for (int i = 0; i < 2; i++) {
+        if (h->ck_key[i]) cudaFree(h->ck_key[i]);
+        if (h->ck_idx[i]) cudaFree(h->ck_idx[i]);
+        h->ck_key[i] = nullptr, h->ck_idx[i] = nullptr;
+      }
+      if (h->ck_tmp) cudaFree(h->ck_tmp);
+      h->ck_tmp = nullptr, h->ck_cap = 0, h->ck_tmp_bytes = 0;
+    };
+    drop();
+    bool ok = true;
+    for (int i = 0; i < 2 && ok; i++)
+      ok = cudaMalloc(&h->ck_key[i], (size_t)nz * sizeof(unsigned)) == cudaSuccess &&
+           cudaMalloc(&h->ck_idx[i], (size_t)nz * sizeof(long long)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->ck_tmp, need) == cudaSuccess;
+    if (!ok) {  // no room for 24 bytes per zone: burn in index order
+      (void)cudaGetLastError();
+      drop();
+      return BZ_OK;
+    }
+    h->ck_cap = nz, h->ck_tmp_bytes = need;
+  }
+  const unsigned blocks = (unsigned)((nz + 255) / 256);
+  bz::cost_key_kernel<<<blocks, 256, 0, st>>>(h->dev, nz, ld, rho, T, X, h->ck_key[0], h->ck_idx[0]);
+  BZ_CUDA(cudaGetLastError());
+  size_t bytes = h->ck_tmp_bytes;
+  BZ_CUDA(cub::DeviceRadixSort::SortPairsDescending(h->ck_tmp, bytes, h->ck_key[0], h->ck_key[1], h->ck_idx[0], h->ck_idx[1],
+                                                    (int)nz, 16, 32, st));
+  *order = h->ck_idx[1];
+  return BZ_OK;
+}
+
 // one launch over nz zones whose rows are `ld` doubles apart; reset_counters = false keeps the event
 // counters of the handle running (the later chunks of burn_zones_host)
 static int launch_burn(const bz_net *h, int64_t nz, int64_t ld, const double *rho, const double *T, const double *X,
@@ -517,7 +585,17 @@ static int launch_burn(const bz_net *h, int64_t nz, int64_t ld, const double *rh
   a.T_out = T_out; a.X_out = X_out; a.nsteps = nsteps;
   a.queue = h->d_scratch; a.counters = h->d_scratch + 1;
   a.mxstep = h->mxstep; a.mxnef = h->mxnef; a.mxncf = h->mxncf;
-  a.static_sched = h->static_sched;
+  a.static_sched = (h->static_sched == 1);
+  a.order = h->order;
+  {
+    // the library's own cost order (a caller's order wins); pointless when the grid takes every zone at once
+    const long long resident = use_quad(h) ? (long long)(h->policy == 1 ? h->quad_grid_reuse : h->quad_grid) * (h->quad->block / 4)
+                                           : (long long)(h->policy == 1 ? h->grid_reuse : h->grid) * (h->coop_threads / h->variant->lanes);
+    if (a.order == nullptr && h->static_sched == 2 && nz > resident) {
+      const int orc = cost_order(h, nz, ld, rho, T, X, st, &a.order);
+      if (orc != BZ_OK) return orc;
+    }
+  }
   if (use_quad(h)) {
     bz::QuadNet qn;
     qn.coef = h->d_quad_coef;
@@ -554,6 +632,8 @@ int burn_zones_src(const bz_net *h, int64_t nz, const double *rho, const double 
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
   if ((src_T == nullptr) != (src_X == nullptr)) return BZ_ERR_NULL;
   if (h->policy == 1 && h->ext) return BZ_ERR_UNSUPPORTED;  // no kept-matrix instantiation with exponents / EOS
+  if (h->order != nullptr && h->order_nz != nz) return BZ_ERR_SIZE;  // the order was given for another batch size
+  if (h->order != nullptr && h->static_sched == 1) return BZ_ERR_UNSUPPORTED;  // the order is the queue's
   const int drc = check_device(h);
   if (drc != BZ_OK) return drc;
   return launch_burn(h, nz, nz, rho, T, X, src_T, src_X, dt, rtol, atol, T_out, X_out, nsteps,
@@ -581,6 +661,7 @@ int burn_zones_host(bz_net *h, int64_t nz, const double *rho, const double *T, c
   if (nz == 0) return BZ_OK;
   if (!rho || !T || !X || !T_out || !X_out || !nsteps) return BZ_ERR_NULL;
   if (h->policy == 1 && h->ext) return BZ_ERR_UNSUPPORTED;
+  if (h->order != nullptr) return BZ_ERR_UNSUPPORTED;  // the host path burns in chunks: no order over the batch
   const int drc = check_device(h);
   if (drc != BZ_OK) return drc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -718,6 +799,7 @@ extern "C" int burn_zones_static(const bz_net_desc *d, int64_t nz, const double 
   a.counters = reinterpret_cast<unsigned long long *>(base) + 1;
   a.mxstep = bz::MXSTEP; a.mxnef = bz::MXNEF; a.mxncf = bz::MXNCF;
   a.static_sched = 0;
+  a.order = nullptr;
   const long long groups_needed = (nz + gpb - 1) / gpb;
   const long long full = (long long)sd->sms * bps;
   const int grid = (int)(groups_needed < full ? groups_needed : full);

@@ -25,7 +25,7 @@ def _record(tag, stats):
         fh.write(json.dumps(dict(tag=tag, **stats)) + "\n")
 
 
-def _burn(net_d, rho, T, X, dt, rtol, atol, kind, src=None, limits=None, schedule="queue"):
+def _burn(net_d, rho, T, X, dt, rtol, atol, kind, src=None, limits=None, schedule="cost"):
     import torch
     import paper_1711_06203_b200 as bz
     dev = torch.device("cuda:0")
