@@ -98,8 +98,10 @@ int net_create(const bz_net_desc *desc, bz_net **out);
  *                    -4  invalid input zone (non-finite, rho <= 0 or T <= 0): outputs = inputs
  *                  failed zones hold the last accepted state; they do not fail the call.
  *   cuda_stream    cudaStream_t (as void*) on which all work is enqueued
- * A handle owns one work-queue counter and one set of counters: calls on the SAME handle must be
- * ordered (same stream, or synchronised); use one handle per concurrent stream.
+ * A handle owns one work-queue counter, one set of counters and, under the default schedule, the buffers of
+ * the queue's cost order (24 bytes per zone, allocated at the first call and when a batch is larger than any
+ * before: bz_set_schedule): calls on the SAME handle must be ordered (same stream, or synchronised); use one
+ * handle per concurrent stream.
  */
 int burn_zones(const bz_net *net, int64_t nz, const double *rho, const double *T, const double *X,
                double dt, double rtol, double atol, double *T_out, double *X_out, int32_t *nsteps,
