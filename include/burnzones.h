@@ -191,12 +191,13 @@ int bz_select_kernel(bz_net *net, int kind);
  *   kind 0: the queue hands the zones out in index order.
  *   kind 1: static round-robin assignment (group g burns zones g, g + G, g + 2G, ...), kept only so that the
  *          benefit of the queue can be MEASURED (bench.py --static-schedule).
- * Every zone's result is bit-identical under all three; only the time differs. */
+ * Every zone's result is bit-identical under all three; only the time differs.  Other kinds: BZ_ERR_SIZE. */
 int bz_set_schedule(bz_net *net, int kind);
 
 /* A caller's own ORDER for the work queue, instead of the library's cost key (e.g. the step counts of the
- * previous hydro step's burn, which the library cannot know).  order: DEVICE pointer to nz int64 entries, a permutation of 0 .. nz-1 -- the q-th zone
- * taken from the queue is zone order[q] -- or NULL (with nz = 0) to return to the handle's schedule.  The
+ * previous hydro step's burn, which the library cannot know).  order: DEVICE pointer to nz int64 entries, a
+ * permutation of 0 .. nz-1 -- the q-th zone taken from the queue is zone order[q] -- or NULL (with nz = 0) to
+ * return to the handle's schedule.  The
  * library keeps the pointer, not a copy: the array is the caller's and must stay valid and unchanged until
  * the burns that use it have completed; it applies to every later burn_zones / burn_zones_src call of this
  * handle, whose nz must equal the nz given here (else BZ_ERR_SIZE); burn_zones_host and the static schedule
